@@ -1,0 +1,329 @@
+"""Grid-level pins of the oracle (BASELINE.json north_star list):
+uniform states and flat space in disguise, SRMHD reduction, exact conservation, closed-form Alfven wave
+with measured convergence order, TOV equilibrium, divergence level, shock-tube symmetries, hydro limit.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import Oracle, OracleParams
+
+
+def make(w, **over):
+    kw = dict(w.params)
+    kw.update(over)
+    o = Oracle(w.n, w.h, w.bc, OracleParams.default(**kw))
+    o.set_metric(w.alpha, w.beta3, w.gamma6)
+    o.set_primitives(w.prim8)
+    return o
+
+
+def l1(a, b):
+    return np.abs(a - b).sum() / a.size
+
+
+# ---- P3: a uniform state is a fixed point on a constant, non-trivial metric ---------------------
+@pytest.mark.parametrize("cleaning", [0, 1])
+def test_uniform_state_constant_metric_is_fixed_point(cleaning):
+    n = (12, 10, 8)
+    a, b, g = wl.constant_metric(n)
+    prim = np.zeros((8, n[2], n[1], n[0]))
+    vals = [0.7, 0.2, -0.3, 0.1, 0.4, 0.3, -0.5, 0.2]
+    for i, v in enumerate(vals):
+        prim[i] = v
+    par = OracleParams.default(gamma_ad=5.0 / 3.0, cleaning=cleaning)
+    o = Oracle(n, (0.1, 0.13, 0.07), (0, 0, 0), par)
+    o.set_metric(a, b, g)
+    o.set_primitives(prim)
+    rhs = o.get_rhs()
+    U = o.get_conserved()
+    scale = np.abs(U).max() / 0.07
+    assert np.abs(rhs).max() <= 1e-13 * scale
+    o.step(0.01, 5)
+    out = o.get_primitives()
+    for i, v in enumerate(vals):
+        assert np.abs(out[i] - v).max() <= 1e-12
+
+
+# ---- P5: special-relativistic reduction: Minkowski sources vanish exactly -----------------------
+def test_minkowski_rhs_is_pure_flux_divergence():
+    """alpha=1, beta=0, gamma=delta: the RHS is the telescoping flux difference plus the -kappa psi
+    damping only: its sum over a periodic box is exactly the round-off of the telescoping sum."""
+    w = wl.alfven_wave(16)
+    o = make(w)
+    o.substeps(w.dt, 2)      # psi becomes non-zero
+    rhs = o.get_rhs()
+    for q in range(8):
+        assert abs(rhs[q].sum()) <= 1e-11 * np.abs(rhs[q]).sum() + 1e-13
+    psi = o.get_psi()
+    assert np.isclose(rhs[8].sum(), -w.params["kappa"] * psi.sum(), rtol=1e-9, atol=1e-12)
+
+
+# ---- P4: flat space in disguise -----------------------------------------------------------------
+def _disguised(w, alpha, s, beta):
+    """The same Minkowski problem in coordinates T = t/alpha, X^i = x^i/s_i - beta^i T: constant
+    lapse alpha, shift beta^i, gamma = diag(s_i^2); vector components scale by 1/s_i."""
+    n = w.n
+    a = np.full_like(w.alpha, alpha)
+    b = np.zeros_like(w.beta3)
+    g = np.zeros_like(w.gamma6)
+    for i in range(3):
+        b[i] = beta[i]
+    g[0], g[3], g[5] = s[0] ** 2, s[1] ** 2, s[2] ** 2
+    prim = w.prim8.copy()
+    for i in range(3):
+        prim[1 + i] /= s[i]
+        prim[5 + i] /= s[i]
+    h = tuple(w.h[i] / s[i] if n[i] > 1 else w.h[i] for i in range(3))
+    return a, b, g, prim, h
+
+
+def test_flat_space_in_disguise_rescaling_is_roundoff_exact():
+    w = wl.alfven_wave(12)
+    alpha, s = 0.8, (1.5, 0.7, 1.2)
+    a, b, g, prim, h = _disguised(w, alpha, s, (0, 0, 0))
+    # kappa is a rate per unit proper time of the normal observers: unchanged
+    o1 = make(w)
+    o2 = Oracle(w.n, h, w.bc, OracleParams.default(**w.params))
+    o2.set_metric(a, b, g)
+    o2.set_primitives(prim)
+    o1.step(w.dt, 6)
+    o2.step(w.dt / alpha, 6)
+    p1, p2 = o1.get_primitives(), o2.get_primitives()
+    for i in range(3):
+        p2[1 + i] *= s[i]
+        p2[5 + i] *= s[i]
+    assert np.abs(p1 - p2).max() <= 5e-13
+    d1, d2 = o1.diagnostics(), o2.diagnostics()
+    vol = s[0] * s[1] * s[2]
+    assert np.isclose(d1["sumD"], d2["sumD"], rtol=1e-12)      # sqrt(gamma) dX dY dZ = dx dy dz
+    assert np.isclose(d1["sumTau"], d2["sumTau"], rtol=1e-12)
+    assert vol > 0
+
+
+@pytest.mark.parametrize("nx", [32])
+def test_flat_space_in_disguise_with_shift_follows_exact_solution(nx):
+    """With a constant shift the coordinates slide over the flat ones, so the discrete scheme is not
+    identical; the result must still follow the exact (mapped) Alfven wave at truncation level, and
+    converge: this fixes the sign and placement of every beta^i term in fluxes and wave speeds."""
+    errs = {}
+    for n1 in (nx, 2 * nx):
+        w = wl.alfven_wave(n1, direction="x")
+        alpha, s = 0.9, (1.25, 1.0, 1.0)
+        T_end = w.extra["period"] / alpha
+        # choose beta^x so the slide over T_end is a whole number of cells at both resolutions
+        beta = (4 * (1.0 / s[0] / nx) / T_end, 0.0, 0.0)      # 4 coarse cells = 8 fine cells
+        a, b, g, prim, h = _disguised(w, alpha, s, beta)
+        o = Oracle(w.n, h, w.bc, OracleParams.default(**w.params))
+        o.set_metric(a, b, g)
+        o.set_primitives(prim)
+        nst = w.nsteps * 2
+        o.step(T_end / nst, nst)
+        p = o.get_primitives()
+        p[1] *= s[0]; p[5] *= s[0]
+        # exact: after one flat period the wave is back; new-coordinate cell X sees x = s (X + beta T)
+        shift = int(round(beta[0] * T_end / h[0]))
+        assert abs(beta[0] * T_end / h[0] - shift) < 1e-9
+        exact = np.roll(w.prim8, -shift, axis=3)
+        errs[n1] = max(l1(p[q], exact[q]) for q in (2, 3, 6, 7))
+        assert l1(p[0], exact[0]) < 1e-2 and errs[n1] < 0.05, (l1(p[0], exact[0]), errs)
+    order = np.log2(errs[nx] / errs[2 * nx])
+    assert order > 1.6, (errs, order)
+
+
+# ---- P6: exact conservation in periodic Minkowski boxes -----------------------------------------
+@pytest.mark.parametrize("cleaning", [0, 1])
+def test_conservation_periodic_minkowski(cleaning):
+    w = wl.alfven_wave(16)
+    rng = np.random.default_rng(8)
+    w.prim8[0] *= 1 + 0.3 * rng.uniform(-1, 1, w.prim8[0].shape)      # make it non-trivial
+    w.prim8[4] *= 1 + 0.3 * rng.uniform(-1, 1, w.prim8[0].shape)
+    o = make(w, cleaning=cleaning)
+    d0 = o.diagnostics()
+    o.step(w.dt, 34)     # 102 substeps
+    d1 = o.diagnostics()
+    for k in ("sumD", "sumTau", "sumBx", "sumBy", "sumBz"):
+        assert abs(d1[k] - d0[k]) <= 1e-13 * abs(d0[k]), k
+    for k in ("sumSx", "sumSy", "sumSz"):
+        assert abs(d1[k] - d0[k]) <= 1e-13 * max(abs(d0[k]), d0["sumTau"]), k
+    assert d1["c2p_fail"] == 0 and d1["atm_reset"] == 0
+
+
+# ---- P8: closed-form circularly polarised Alfven wave, convergence order ------------------------
+def test_alfven_speed_closed_form():
+    """v_A from the Alfven characteristic condition: omega/k solves
+    (rho h + b^2) W^2 (v_A - v_par)^2 = (B_par/W + W (B.v)(v_A - v_par))^2 ... for the circular wave this
+    reduces to the quadratic  B0^2 (1 + eta^2 v_A^2)/... ; here we simply check the survey's number
+    against the defining relation  v_A^2 (rho h + B0^2 (1 + eta^2 (1 - v_A^2))) = B0^2 (1 - eta^2 v_A^2 ...)
+    in its solved form: (3 - sqrt 5)/2 is the root of  x^2 - 3x + 1 = 0  that is < 1."""
+    va = wl.ALFVEN_VA
+    assert abs(va * va - 3 * va + 1) < 1e-15 and 0 < va < 1
+    # defining condition for rho=p=B0=eta=1, Gamma=4/3: transverse v = -va*eta*e, B_t = eta*e.
+    # comoving b^2 = B^2/W^2 + (B.v)^2, total enthalpy E = rho h + b^2, Alfven speed along n:
+    # va = B_n / (sqrt(E) W ... ) evaluated from the state itself:
+    rho, p, B0, eta, G = 1.0, 1.0, 1.0, 1.0, 4.0 / 3.0
+    vt = va * eta
+    W = 1 / np.sqrt(1 - vt * vt)
+    Bv = -eta * B0 * vt
+    B2 = B0 * B0 * (1 + eta * eta)
+    b2 = B2 / W ** 2 + Bv ** 2
+    E = rho * (1 + G / (G - 1) * p / rho) + b2
+    bn = B0 / W                       # b^n (v_n = 0)
+    u0 = W
+    # Alfven characteristic: lambda = (b^n +- sqrt(E) u^n)/(b^0 +- sqrt(E) u^0), u^n = 0, b^0 = W Bv
+    lam = bn / (W * Bv + np.sqrt(E) * u0)
+    lam2 = bn / (W * Bv - np.sqrt(E) * u0)
+    assert min(abs(abs(lam) - va), abs(abs(lam2) - va)) < 1e-14
+
+
+def test_alfven_wave_convergence_1d():
+    errs = []
+    for nx in (32, 64, 128):
+        w = wl.alfven_wave(nx, direction="x")
+        o = make(w)
+        o.step(w.dt, w.nsteps)
+        p = o.get_primitives()
+        errs.append(max(l1(p[q], w.prim8[q]) for q in (2, 3, 6, 7)))
+        d = o.diagnostics()
+        assert d["c2p_fail"] == 0 and d["atm_reset"] == 0
+    o1, o2 = np.log2(errs[0] / errs[1]), np.log2(errs[1] / errs[2])
+    assert errs[2] < 2e-3
+    assert o1 > 1.7 and o2 > 1.7, (errs, o1, o2)
+
+
+def test_alfven_wave_convergence_3d_diagonal():
+    errs = []
+    for nx in (16, 32):
+        w = wl.alfven_wave(nx)
+        o = make(w)
+        o.step(w.dt, w.nsteps)
+        p = o.get_primitives()
+        errs.append(max(l1(p[q], w.prim8[q]) for q in (1, 2, 3, 5, 6, 7)))
+    order = np.log2(errs[0] / errs[1])
+    assert order > 1.5, (errs, order)
+
+
+# ---- P11: TOV ------------------------------------------------------------------------------------
+def test_tov_ode_check_values():
+    """Golden values: tests/golden/tov_check_values.txt (rtol 1e-12 integration)."""
+    tov = wl.tov_solve()
+    path = os.path.join(os.path.dirname(__file__), "golden", "tov_check_values.txt")
+    gold = {}
+    for line in open(path):
+        if line.strip() and not line.startswith("#"):
+            k, v = line.split()[:2]
+            gold[k] = float(v)
+    assert np.isclose(tov["M"], gold["M"], rtol=2e-5)
+    assert np.isclose(tov["R"], gold["R_areal"], rtol=2e-5)
+    assert np.isclose(tov["Riso"], gold["R_iso"], rtol=2e-5)
+    assert np.isclose(tov["alpha_c"], gold["alpha_centre"], rtol=2e-5)
+    assert np.isclose(tov["alpha_s"], gold["alpha_surface"], rtol=2e-5)
+    assert np.isclose(tov["p_c"], gold["p_max"], rtol=1e-4)
+    # exterior matching: alpha_s = sqrt(1 - 2M/R) and R = Riso (1 + M/(2 Riso))^2 (Schwarzschild)
+    assert np.isclose(tov["alpha_s"] ** 2, 1 - 2 * tov["M"] / tov["R"], rtol=1e-12)
+    assert np.isclose(tov["R"], tov["Riso"] * (1 + tov["M"] / (2 * tov["Riso"])) ** 2, rtol=1e-10)
+
+
+def test_tov_star_is_an_equilibrium_of_the_scheme():
+    """Omega = 0, B = 0: the acceleration a fluid element picks up in one substep is pure truncation
+    error.  In L1 over a smooth shell it converges at second order (the max norm does not: MC clips the
+    central extremum), and it is tiny against the gravitational acceleration M/r^2 ~ 0.04 that the
+    source terms must balance against the pressure gradient on this genuinely curved metric."""
+    tov = wl.tov_solve()
+    res = []
+    for nx in (24, 48):
+        w = wl.tov_star(nx, half_width=12.0, Omega=0.0, Bmax=0.0, tov=tov)
+        o = make(w)
+        o.substeps(w.dt, 1)
+        p = o.get_primitives()
+        x, _ = wl.centres(nx, -12.0, 12.0)
+        Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+        r = np.sqrt(X * X + Y * Y + Z * Z)
+        shell = (r >= 2.0) & (r < 6.0)
+        acc = np.sqrt((p[1:4] ** 2).sum(axis=0)) / w.dt
+        res.append(acc[shell].mean())
+    assert res[1] < res[0] / 3.0, res
+    assert res[1] < 0.04 / 50, res
+
+
+# ---- P12: divergence level -----------------------------------------------------------------------
+def test_divergence_cleaning_reduces_divB():
+    w = wl.alfven_wave(16)
+    rng = np.random.default_rng(9)
+    w.prim8[5] += 0.2 * np.exp(-((np.arange(16)[None, None, :] - 8) ** 2) / 8.0)   # a monopole layer
+    o_off, o_on = make(w, cleaning=0), make(w, cleaning=1, kappa=5.0)
+    d0 = o_on.diagnostics()
+    assert d0["divB_L1"] > 1e-2
+    for o in (o_off, o_on):
+        o.step(w.dt, 60)
+    doff, don = o_off.diagnostics(), o_on.diagnostics()
+    assert don["divB_L1"] < 0.5 * doff["divB_L1"]
+    assert don["divB_L1"] < 0.5 * d0["divB_L1"]
+    del rng
+
+
+def test_tov_initial_field_is_divergence_free_to_roundoff():
+    w = wl.tov_star(24, half_width=12.0)
+    o = make(w)
+    d = o.diagnostics()
+    Bscale = 1e-4 / w.h[0]
+    assert d["divB_max"] <= 1e-12 * Bscale
+
+
+# ---- P13: shock tube ----------------------------------------------------------------------------
+def test_shock_tube_bx_constant_mirror_symmetry_and_self_convergence():
+    w = wl.shock_tube(200)
+    o = make(w)
+    o.step(w.dt, w.nsteps)
+    p = o.get_primitives()
+    assert np.abs(p[5] - 0.5).max() <= 1e-13
+    assert np.abs(o.get_psi()).max() <= 1e-13
+    assert np.all(p[7] == 0.0) and np.all(p[3] == 0.0)
+    wm = wl.shock_tube(200, mirror=True)
+    om = make(wm)
+    om.step(wm.dt, wm.nsteps)
+    pm = om.get_primitives()
+    assert np.array_equal(pm[0][..., ::-1], p[0]) and np.array_equal(pm[4][..., ::-1], p[4])
+    assert np.array_equal(pm[1][..., ::-1], -p[1])
+    assert np.array_equal(pm[6][..., ::-1], p[6])       # left state has By=+1 in both set-ups
+    # along y: same numbers with axes permuted (direction-dependent code paths)
+    wy = wl.shock_tube(200, axis=1)
+    oy = make(wy)
+    oy.step(wy.dt, wy.nsteps)
+    py = oy.get_primitives()
+    assert np.array_equal(py[0].ravel(), p[0].ravel())
+    assert np.array_equal(py[2].ravel(), p[1].ravel()) and np.array_equal(py[7].ravel(), p[6].ravel())
+    # first-order self-convergence in L1 (the solution has discontinuities)
+    sols = {200: p[0].ravel()}
+    for nx in (400, 800):
+        wn = wl.shock_tube(nx)
+        on = make(wn)
+        on.step(wn.dt, wn.nsteps)
+        sols[nx] = on.get_primitives()[0].ravel()
+    c400 = sols[400].reshape(-1, 2).mean(axis=1)
+    c800 = sols[800].reshape(-1, 4).mean(axis=1)
+    e1, e2 = l1(sols[200], c400), l1(c400, c800)
+    assert e2 < 0.75 * e1 and e1 < 0.02
+    # physical sanity: states between the initial extremes, waves have left the centre
+    assert p[0].max() <= 1.0 + 1e-3 and p[0].min() >= 0.125 - 1e-3
+
+
+# ---- P14: hydro limit ---------------------------------------------------------------------------
+def test_hydro_limit_sod_stays_one_dimensional_and_unmagnetised():
+    n = (64, 4, 4)
+    x, dx = wl.centres(64, -0.5, 0.5)
+    prim = np.zeros((8, 4, 4, 64))
+    prim[0] = np.where(x < 0, 1.0, 0.125)
+    prim[4] = np.where(x < 0, 1.0, 0.1)
+    a, b, g = wl.minkowski(n)
+    par = OracleParams.default(gamma_ad=5.0 / 3.0)     # PAPER.md:286 Sod set-up
+    o = Oracle(n, (dx, dx, dx), (1, 0, 0), par)
+    o.set_metric(a, b, g)
+    o.set_primitives(prim)
+    o.step(0.4 * dx, 40)
+    p = o.get_primitives()
+    assert np.all(p[5:8] == 0.0) and np.all(p[2:4] == 0.0)
+    assert np.array_equal(p[:, 0, 0, :], p[:, 3, 2, :])
+    assert p[1].max() > 0.1     # the flow has started
