@@ -307,7 +307,7 @@ def test_shock_tube_bx_constant_mirror_symmetry_and_self_convergence():
     e1, e2 = l1(sols[200], c400), l1(c400, c800)
     assert e2 < 0.75 * e1 and e1 < 0.02
     # physical sanity: states between the initial extremes, waves have left the centre
-    assert p[0].max() <= 1.0 + 1e-3 and p[0].min() >= 0.125 - 1e-3
+    assert p[0].max() <= 1.0 + 1e-3 and p[0].min() >= 0.1   # the right fast rarefaction dips below 0.125
 
 
 # ---- P14: hydro limit ---------------------------------------------------------------------------
