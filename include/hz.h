@@ -1,0 +1,135 @@
+/* hz.h -- C ABI of the B200-native HORIZON GRMHD update (libhz.so).
+ *
+ * What the library does: it advances ideal GRMHD in 3+1 conservative form on a uniform Cartesian
+ * mesh in a fixed, given spacetime by method-of-lines Runge-Kutta substeps.  One substep is the
+ * pipeline of PAPER.md:74-80 (section 2.2): reconstruct the primitives at the faces, evaluate
+ * left/right fluxes and maximal wave speeds, take an approximate (HLLE) Riemann flux, difference the
+ * fluxes and add the local geometric source terms of PAPER.md:54 (eq. 2), combine the Runge-Kutta
+ * stage, recover the primitives by Newton-Raphson and refill the ghost zones.  The named
+ * ingredients are those of PAPER.md:128 (section 3.2): HLLE, TVD reconstruction with the MC limiter,
+ * third-order Runge-Kutta, Newton-Raphson primitive recovery, hyperbolic divergence cleaning.  Every
+ * discrete formula the paper does not print is a reading listed in DESIGN.md (R1-R22).
+ *
+ * Every step of that path runs in hand-written CUDA kernels for sm_100a, in fp64 or fp32 (one dtype
+ * per context).  There is NO CPU fallback: without a CUDA device every compute entry point returns
+ * HZ_ECUDA.
+ *
+ * Conventions
+ *   Layout    Every field array is INTERIOR-ONLY, nx*ny*nz elements per plane, x fastest
+ *             (PAPER.md:152), planes concatenated.  Element type = the context dtype
+ *             (HZ_F32: float, HZ_F64: double).  The library pads, adds ghost zones and fills
+ *             them itself.
+ *   Pointers  Every `const void*` / `void*` field argument may be a HOST pointer (pageable or
+ *             pinned) or a DEVICE pointer; the library resolves which with
+ *             cudaPointerGetAttributes and copies.  The caller owns these buffers before and
+ *             after the call; the library keeps no reference to them.
+ *   Stream    All device work of a context is enqueued on its stream (default: the legacy default
+ *             stream; hz_set_stream changes it).  hz_step / hz_substeps are ASYNCHRONOUS: they
+ *             return once the work is enqueued.  hz_set_*, hz_get_* and hz_diagnostics
+ *             synchronise the stream before returning.
+ *   Errors    Every call returns an int: HZ_OK (0) or a negative code.  No exception crosses
+ *             the ABI and the library never exits the process.
+ *   Units     G = c = 1; B^i is the Eulerian-observer magnetic field with 1/sqrt(4 pi) absorbed
+ *             (b^2 adds to rho h without a 4 pi).  Velocities at the boundary are the Eulerian
+ *             3-velocity v^i (contravariant); internally the library stores W v^i
+ *             (footnote 3).
+ */
+#ifndef HZ_H
+#define HZ_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hz_ctx hz_ctx; /* opaque; created by hz_create, freed by hz_destroy */
+
+enum { HZ_F32 = 0, HZ_F64 = 1 };
+enum { HZ_BC_PERIODIC = 0, HZ_BC_OUTFLOW = 1 }; /* per axis */
+enum { HZ_OK = 0, HZ_EINVAL = -1, HZ_ENOMEM = -2, HZ_ECUDA = -3, HZ_ESTATE = -4 };
+
+/* Uniform Cartesian mesh.  An axis with one cell is inactive: no ghost zones, no
+ * sweep, no derivative along it (two-dimensional meshes). */
+typedef struct { int nx, ny, nz; double dx, dy, dz; int bc[3]; } hz_grid;
+
+typedef struct {
+  double gamma_ad;        /* ideal-gas adiabatic index Gamma (> 1)                              */
+  double rho_atm, p_atm;  /* atmosphere values; also the floors of the face states              */
+  double atm_tol;         /* a cell is reset to atmosphere if rho < rho_atm*(1+atm_tol)         */
+  int    cleaning;        /* 0: psi frozen at 0; 1: hyperbolic divergence cleaning */
+  double kappa;           /* cleaning damping rate                                              */
+  int    c2p_maxit;       /* Newton iteration cap of the primitive recovery                     */
+  double c2p_tol;         /* converged when |dZ| <= c2p_tol*Z; <= 0 selects the dtype default   */
+                          /* (1e-13 for HZ_F64, 1e-6 for HZ_F32)                                */
+} hz_params;
+
+/* Global reductions, all accumulated in fp64. */
+typedef struct {
+  double sumD, sumSx, sumSy, sumSz, sumTau;  /* sum over interior cells of sqrt(gamma)*(..)*dx*dy*dz */
+  double sumBx, sumBy, sumBz, sumPsi;
+  double divB_max, divB_L1;                  /* centred div(sqrt(gamma) B)/sqrt(gamma): max, mean |.| */
+  double max_speed_over_dx;                  /* max over cells, axes of max(|lam+|,|lam-|)/dx_d       */
+  long long c2p_fail, atm_reset, p_floor;    /* cumulative since hz_set_primitives                    */
+  int c2p_maxit_seen;
+} hz_diag;
+
+/* Fill *p with the defaults: Gamma = 4/3, atmosphere 1e-12 / 1e-14, atm_tol 1e-3, cleaning on,
+ * kappa = 1, 30 Newton iterations, c2p_tol = 0 (dtype default).  HZ_EINVAL if p is NULL. */
+int hz_default_params(hz_params* p);
+
+/* Bytes of device memory one context of this grid and dtype needs (all resident fields: metric,
+ * two primitive sets, conserved, conserved at the step start, staging and reduction scratch).
+ * HZ_EINVAL on a bad grid or dtype.  Needs no GPU. */
+int hz_state_bytes(const hz_grid* grid, int dtype, size_t* bytes);
+
+/* Create a context.  `device_buffer` is either NULL (the library allocates hz_state_bytes with
+ * cudaMalloc and frees it in hz_destroy) or a caller-owned DEVICE buffer of at least hz_state_bytes
+ * bytes, 256-byte aligned (e.g. a torch.uint8 tensor's data_ptr()), which must outlive the context.
+ * `params` may be NULL (defaults).  Errors: HZ_EINVAL (bad grid: n < 1, 1 < n < 2 along an axis,
+ * spacing <= 0, unknown bc or dtype, Gamma <= 1, maxit < 1), HZ_ECUDA (no device / CUDA failure),
+ * HZ_ENOMEM. */
+int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* device_buffer, hz_ctx** out);
+int hz_destroy(hz_ctx* ctx);
+
+/* Use `cuda_stream` (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream; NULL = default
+ * stream) for all later work of this context. */
+int hz_set_stream(hz_ctx* ctx, void* cuda_stream);
+
+/* Fixed spacetime: lapse `alpha` (1 plane), shift `beta3` (beta^x, beta^y, beta^z:
+ * 3 planes), spatial metric `gamma6` (xx, xy, xz, yy, yz, zz: 6 planes).  Ghost zones are filled by
+ * periodic wrap or by copying the nearest interior cell (outflow axes).  HZ_EINVAL if any value is
+ * non-finite, alpha <= 0 or gamma_ij is not positive definite.  Invalidates the primitives. */
+int hz_set_metric(hz_ctx* ctx, const void* alpha, const void* beta3, const void* gamma6);
+
+/* Initial data in primitive variables: `prim8` = rho, v^x, v^y, v^z, p, B^x, B^y, B^z
+ * (8 planes).  Runs prim->cons and the ghost fill; sets psi = 0, the Runge-Kutta stage
+ * to 0 and the counters of hz_diag to 0.  HZ_ESTATE before hz_set_metric; HZ_EINVAL if a value is
+ * non-finite, rho <= 0, p < 0 or v^2 >= 1. */
+int hz_set_primitives(hz_ctx* ctx, const void* prim8);
+
+/* Advance n full third-order Runge-Kutta steps (= 3n substeps) with the fixed step dt
+ * (PAPER.md:128, 238).  Asynchronous.  HZ_ESTATE before metric and primitives are set or in the
+ * middle of a step (after hz_substeps with a count not divisible by 3); HZ_EINVAL if dt <= 0, n < 0.
+ * Failed primitive recoveries are not errors: the cell is reset to atmosphere and counted. */
+int hz_step(hz_ctx* ctx, double dt, int n);
+/* Advance `nsub` Runge-Kutta substeps, continuing from the current stage.  Asynchronous. */
+int hz_substeps(hz_ctx* ctx, double dt, int nsub);
+
+/* Current primitives in the layout of hz_set_primitives (v^i = W v^i / W), the cleaning scalar psi
+ * (1 plane) and the densitised conserved variables sqrt(gamma)*(D, S_x, S_y, S_z, tau, B^x, B^y,
+ * B^z, psi) (9 planes). */
+int hz_get_primitives(hz_ctx* ctx, void* prim8);
+int hz_get_psi(hz_ctx* ctx, void* psi);
+int hz_get_conserved(hz_ctx* ctx, void* cons9);
+
+/* Global reductions over the current state.  Synchronises the stream. */
+int hz_diagnostics(hz_ctx* ctx, hz_diag* out);
+
+/* Number of kernels this context has launched since hz_create (bench.py's gpu_launches). */
+long long hz_launch_count(const hz_ctx* ctx);
+
+const char* hz_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

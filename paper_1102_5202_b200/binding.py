@@ -1,0 +1,232 @@
+"""ctypes binding of libhz.so.  Same names as include/hz.h; argument marshalling only."""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+HZ_F32, HZ_F64 = 0, 1
+HZ_BC_PERIODIC, HZ_BC_OUTFLOW = 0, 1
+HZ_OK, HZ_EINVAL, HZ_ENOMEM, HZ_ECUDA, HZ_ESTATE = 0, -1, -2, -3, -4
+
+# every symbol include/hz.h declares (tests check the library exports each of them)
+SYMBOLS = ["hz_default_params", "hz_state_bytes", "hz_create", "hz_destroy", "hz_set_stream", "hz_set_metric",
+           "hz_set_primitives", "hz_step", "hz_substeps", "hz_get_primitives", "hz_get_psi", "hz_get_conserved",
+           "hz_diagnostics", "hz_launch_count", "hz_strerror"]
+
+
+class HzGrid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double), ("bc", C.c_int * 3)]
+
+
+class HzParams(C.Structure):
+    _fields_ = [("gamma_ad", C.c_double), ("rho_atm", C.c_double), ("p_atm", C.c_double), ("atm_tol", C.c_double),
+                ("cleaning", C.c_int), ("kappa", C.c_double), ("c2p_maxit", C.c_int), ("c2p_tol", C.c_double)]
+
+    @classmethod
+    def default(cls, **kw):
+        p = cls()
+        lib().hz_default_params(C.byref(p))
+        for k, v in kw.items():
+            if not hasattr(p, k):
+                raise AttributeError(k)
+            setattr(p, k, v)
+        return p
+
+
+class HzDiag(C.Structure):
+    _fields_ = [("sumD", C.c_double), ("sumSx", C.c_double), ("sumSy", C.c_double), ("sumSz", C.c_double),
+                ("sumTau", C.c_double), ("sumBx", C.c_double), ("sumBy", C.c_double), ("sumBz", C.c_double),
+                ("sumPsi", C.c_double), ("divB_max", C.c_double), ("divB_L1", C.c_double),
+                ("max_speed_over_dx", C.c_double), ("c2p_fail", C.c_longlong), ("atm_reset", C.c_longlong),
+                ("p_floor", C.c_longlong), ("c2p_maxit_seen", C.c_int)]
+
+    def asdict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class HzError(RuntimeError):
+    def __init__(self, code, where=""):
+        self.code = code
+        try:
+            msg = lib().hz_strerror(code).decode()
+        except Exception:
+            msg = "?"
+        super().__init__(f"{where}: hz error {code}: {msg}")
+
+
+_lib = None
+
+
+def lib_path():
+    return os.path.join(HERE, "libhz.so")
+
+
+def lib():
+    """Load libhz.so (built in-tree by paper_1102_5202_b200/build.py).  Fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            raise RuntimeError(f"{path} is missing: run `python -m paper_1102_5202_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(path)
+        vp, ip = C.c_void_p, C.c_int
+        L.hz_default_params.argtypes = [C.POINTER(HzParams)]
+        L.hz_state_bytes.argtypes = [C.POINTER(HzGrid), ip, C.POINTER(C.c_size_t)]
+        L.hz_create.argtypes = [C.POINTER(HzGrid), ip, C.POINTER(HzParams), vp, C.POINTER(vp)]
+        L.hz_destroy.argtypes = [vp]
+        L.hz_set_stream.argtypes = [vp, vp]
+        L.hz_set_metric.argtypes = [vp, vp, vp, vp]
+        L.hz_set_primitives.argtypes = [vp, vp]
+        L.hz_step.argtypes = [vp, C.c_double, ip]
+        L.hz_substeps.argtypes = [vp, C.c_double, ip]
+        L.hz_get_primitives.argtypes = [vp, vp]
+        L.hz_get_psi.argtypes = [vp, vp]
+        L.hz_get_conserved.argtypes = [vp, vp]
+        L.hz_diagnostics.argtypes = [vp, C.POINTER(HzDiag)]
+        L.hz_launch_count.argtypes = [vp]
+        L.hz_launch_count.restype = C.c_longlong
+        L.hz_strerror.argtypes = [ip]
+        L.hz_strerror.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _chk(rc, where):
+    if rc != 0:
+        raise HzError(rc, where)
+
+
+def _ptr(a):
+    """Address of a numpy array (host) or a torch tensor (host or device)."""
+    if isinstance(a, np.ndarray):
+        return C.c_void_p(a.ctypes.data)
+    return C.c_void_p(a.data_ptr())  # torch.Tensor
+
+
+class Horizon:
+    """One grid, one dtype.  Arrays in and out have shape (planes, nz, ny, nx), x fastest.
+
+    Inputs may be numpy arrays (host) or torch tensors (host or CUDA) of the context dtype; other
+    float arrays are converted.  `get_*` return numpy arrays unless `out=` (numpy or torch) is given.
+    Device state lives in a torch.uint8 CUDA tensor (PyTorch is used for device memory and streams only).
+    """
+
+    def __init__(self, n, h, bc, dtype="f64", params=None, stream=None, use_torch_memory=True):
+        import torch
+        L = lib()
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the HORIZON update has no CPU fallback")
+        self.n = tuple(int(x) for x in n)
+        self.ncell = self.n[0] * self.n[1] * self.n[2]
+        if dtype in ("f64", "float64", np.float64):
+            self.dtype = HZ_F64
+        elif dtype in ("f32", "float32", np.float32):
+            self.dtype = HZ_F32
+        else:
+            raise ValueError(f"dtype must be 'f64' or 'f32', got {dtype!r}")
+        self.np_dtype = np.float64 if self.dtype == HZ_F64 else np.float32
+        self.grid = HzGrid(self.n[0], self.n[1], self.n[2], float(h[0]), float(h[1]), float(h[2]),
+                           (C.c_int * 3)(*[int(b) for b in bc]))
+        self.params = params if params is not None else HzParams.default()
+        nbytes = C.c_size_t(0)
+        _chk(L.hz_state_bytes(C.byref(self.grid), self.dtype, C.byref(nbytes)), "hz_state_bytes")
+        self.state_bytes = nbytes.value
+        self._buf = None
+        buf_ptr = None
+        if use_torch_memory:
+            self._buf = torch.empty(self.state_bytes + 256, dtype=torch.uint8, device="cuda")
+            base = self._buf.data_ptr()
+            buf_ptr = C.c_void_p((base + 255) // 256 * 256)
+        h_ = C.c_void_p()
+        _chk(L.hz_create(C.byref(self.grid), self.dtype, C.byref(self.params), buf_ptr, C.byref(h_)), "hz_create")
+        self._h = h_
+        if stream is not None:
+            self.set_stream(stream)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().hz_destroy(self._h)
+            self._h = None
+            self._buf = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- marshalling helpers ----
+    def _in(self, a, planes):
+        if isinstance(a, np.ndarray) or not hasattr(a, "data_ptr"):
+            a = np.ascontiguousarray(np.asarray(a), dtype=self.np_dtype)
+        else:
+            import torch
+            td = torch.float64 if self.dtype == HZ_F64 else torch.float32
+            if a.dtype != td or not a.is_contiguous():
+                a = a.to(td).contiguous()
+        size = a.size if isinstance(a, np.ndarray) else a.numel()
+        if size != planes * self.ncell:
+            raise ValueError(f"expected {planes * self.ncell} values, got {size}")
+        return a
+
+    def _out(self, out, planes):
+        if out is None:
+            return np.empty((planes, self.n[2], self.n[1], self.n[0]), dtype=self.np_dtype)
+        size = out.size if isinstance(out, np.ndarray) else out.numel()
+        if size != planes * self.ncell:
+            raise ValueError(f"expected {planes * self.ncell} values, got {size}")
+        return out
+
+    # ---- the C-ABI calls, same names ----
+    def set_stream(self, stream):
+        s = getattr(stream, "cuda_stream", stream)
+        _chk(lib().hz_set_stream(self._h, C.c_void_p(s)), "hz_set_stream")
+
+    def set_metric(self, alpha, beta3, gamma6):
+        a, b, g = self._in(alpha, 1), self._in(beta3, 3), self._in(gamma6, 6)
+        _chk(lib().hz_set_metric(self._h, _ptr(a), _ptr(b), _ptr(g)), "hz_set_metric")
+
+    def set_primitives(self, prim8):
+        a = self._in(prim8, 8)
+        _chk(lib().hz_set_primitives(self._h, _ptr(a)), "hz_set_primitives")
+
+    def step(self, dt, n):
+        _chk(lib().hz_step(self._h, float(dt), int(n)), "hz_step")
+
+    def substeps(self, dt, nsub):
+        _chk(lib().hz_substeps(self._h, float(dt), int(nsub)), "hz_substeps")
+
+    def get_primitives(self, out=None):
+        out = self._out(out, 8)
+        _chk(lib().hz_get_primitives(self._h, _ptr(out)), "hz_get_primitives")
+        return out
+
+    def get_psi(self, out=None):
+        out = self._out(out, 1)
+        _chk(lib().hz_get_psi(self._h, _ptr(out)), "hz_get_psi")
+        return out[0] if isinstance(out, np.ndarray) else out
+
+    def get_conserved(self, out=None):
+        out = self._out(out, 9)
+        _chk(lib().hz_get_conserved(self._h, _ptr(out)), "hz_get_conserved")
+        return out
+
+    def diagnostics(self):
+        d = HzDiag()
+        _chk(lib().hz_diagnostics(self._h, C.byref(d)), "hz_diagnostics")
+        return d.asdict()
+
+    def launch_count(self):
+        return lib().hz_launch_count(self._h)
+
+    @classmethod
+    def from_workload(cls, w, dtype="f64", **kw):
+        """Context for a workloads.Workload, with metric and primitives set."""
+        par = HzParams.default(**w.params)
+        hz = cls(w.n, w.h, w.bc, dtype=dtype, params=par, **kw)
+        hz.set_metric(w.alpha, w.beta3, w.gamma6)
+        hz.set_primitives(w.prim8)
+        return hz

@@ -1,0 +1,421 @@
+// hz_kernels.cuh -- the kernels of one Runge-Kutta substep and of the set/get/diagnostic calls.
+//
+// Substep = k_rhs_update (reconstruction, HLLE fluxes, flux difference, sources, RK combine:
+// PAPER.md:76-80) -> k_con2prim (Newton-Raphson recovery + floors) -> k_fill_ghosts.
+// All kernels are templated on the arithmetic type (double / float).
+#pragma once
+#include "hz_layout.cuh"
+#include "hz_physics.cuh"
+
+namespace hz {
+
+constexpr int BLK = 128;       // threads per block of the per-cell kernels
+constexpr int NDIAG = 16;      // doubles per block partial of the diagnostics reduction
+
+// interior linear index -> (i, j, k), x fastest
+__device__ __forceinline__ void cell_of(const Layout& L, long long t, int& i, int& j, int& k) {
+  i = (int)(t % L.n[0]);
+  long long r = t / L.n[0];
+  j = (int)(r % L.n[1]);
+  k = (int)(r / L.n[1]);
+}
+
+template <typename T>
+__device__ __forceinline__ void load_fields(const T* __restrict__ F, long long fs, long long id, int nf, T* out) {
+#pragma unroll
+  for (int q = 0; q < NM; q++)
+    if (q < nf) out[q] = F[q * fs + id];
+}
+
+// ---- ghost fill (O9 / R15): periodic wrap or zero-gradient copy, any number of fields ---
+template <typename T>
+__global__ void k_fill_ghosts(Layout L, T* __restrict__ F, int nf) {
+  const long long ntot = (long long)L.N[0] * L.N[1] * L.N[2];
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ntot) return;
+  int c[3];
+  c[0] = (int)(t % L.N[0]) - L.g[0];
+  long long r = t / L.N[0];
+  c[1] = (int)(r % L.N[1]) - L.g[1];
+  c[2] = (int)(r / L.N[1]) - L.g[2];
+  int s[3];
+  bool ghost = false;
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    const int n = L.n[d];
+    if (c[d] < 0 || c[d] >= n) {
+      ghost = true;
+      s[d] = L.bc[d] == 0 ? ((c[d] % n) + n) % n : (c[d] < 0 ? 0 : n - 1);
+    } else {
+      s[d] = c[d];
+    }
+  }
+  if (!ghost) return;
+  const long long dst = L.idx(c[0], c[1], c[2]), src = L.idx(s[0], s[1], s[2]);
+  for (int f = 0; f < nf; f++) F[f * L.fs + dst] = F[f * L.fs + src];
+}
+
+// ---- hz_set_metric: interior-only planes -> padded SoA, with validation -------------------------
+template <typename T>
+__global__ void k_pack_metric(Layout L, const T* __restrict__ alpha, const T* __restrict__ beta3,
+                              const T* __restrict__ gamma6, T* __restrict__ met, int* __restrict__ err) {
+  const long long n = L.ncell();
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  int i, j, k;
+  cell_of(L, t, i, j, k);
+  T m[NM];
+  m[0] = alpha[t];
+#pragma unroll
+  for (int a = 0; a < 3; a++) m[1 + a] = beta3[a * n + t];
+#pragma unroll
+  for (int a = 0; a < 6; a++) m[4 + a] = gamma6[a * n + t];
+  T c[6];
+  T det = cofactors(m + GXX, c);
+  bool ok = m[AL] > 0 && det > 0 && m[GXX] > 0 && c[5] > 0;
+#pragma unroll
+  for (int a = 0; a < NM; a++) ok = ok && finite_(m[a]);
+  ok = ok && finite_(det);
+  if (!ok) atomicOr(err, 1);
+  const long long id = L.idx(i, j, k);
+#pragma unroll
+  for (int a = 0; a < NM; a++) met[a * L.fs + id] = m[a];
+}
+
+// ---- hz_set_primitives: (rho, v^i, p, B^i) -> stored primitives (W v^i, psi = 0) and sqrt(gamma) U
+template <typename T>
+__global__ void k_pack_prims(Layout L, Par<T> par, const T* __restrict__ prim8, const T* __restrict__ met,
+                             T* __restrict__ P, T* __restrict__ U, int* __restrict__ err) {
+  const long long n = L.ncell();
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  int i, j, k;
+  cell_of(L, t, i, j, k);
+  const long long id = L.idx(i, j, k);
+  T m[NM];
+  load_fields(met, L.fs, id, NM, m);
+  T a8[8];
+  bool ok = true;
+#pragma unroll
+  for (int q = 0; q < 8; q++) { a8[q] = prim8[q * n + t]; ok = ok && finite_(a8[q]); }
+  T vl[3];
+  lower(m + GXX, a8 + 1, vl);
+  T v2 = dot3(a8 + 1, vl);
+  ok = ok && a8[0] > 0 && !(a8[4] < 0) && v2 < 1;
+  if (!ok) { atomicOr(err, 1); return; }
+  T W = rcp_(sqrt_(1 - v2));
+  T q[NV];
+  q[RHO] = a8[0]; q[PR] = a8[4]; q[PSI] = 0;
+#pragma unroll
+  for (int a = 0; a < 3; a++) { q[UX + a] = W * a8[1 + a]; q[BX + a] = a8[5 + a]; }
+  T w[NV];
+  prim2con(q, m, par, w);
+  T sq = sqrt_det(m + GXX);
+#pragma unroll
+  for (int v = 0; v < NV; v++) { P[v * L.fs + id] = q[v]; U[v * L.fs + id] = sq * w[v]; }
+}
+
+// ---- hz_get_primitives ---------------------------------------------------------------------------
+template <typename T>
+__global__ void k_unpack_prims(Layout L, const T* __restrict__ P, const T* __restrict__ met, T* __restrict__ prim8) {
+  const long long n = L.ncell();
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  int i, j, k;
+  cell_of(L, t, i, j, k);
+  const long long id = L.idx(i, j, k);
+  T g[6], q[NV];
+#pragma unroll
+  for (int a = 0; a < 6; a++) g[a] = met[(GXX + a) * L.fs + id];
+  load_fields(P, L.fs, id, NV, q);
+  T utl[3];
+  lower(g, q + UX, utl);
+  T iW = rcp_(sqrt_(1 + dot3(q + UX, utl)));
+  prim8[0 * n + t] = q[RHO];
+#pragma unroll
+  for (int d = 0; d < 3; d++) prim8[(1 + d) * n + t] = q[UX + d] * iW;
+  prim8[4 * n + t] = q[PR];
+#pragma unroll
+  for (int d = 0; d < 3; d++) prim8[(5 + d) * n + t] = q[BX + d];
+}
+
+// nf padded fields starting at field f0 -> interior-only planes
+template <typename T>
+__global__ void k_unpack_fields(Layout L, const T* __restrict__ F, int f0, int nf, T* __restrict__ out) {
+  const long long n = L.ncell();
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  int i, j, k;
+  cell_of(L, t, i, j, k);
+  const long long id = L.idx(i, j, k);
+  for (int f = 0; f < nf; f++) out[f * n + t] = F[(f0 + f) * L.fs + id];
+}
+
+// ---- a1-a5 for one face: MC reconstruction of the 9 primitives, face metric, HLLE ---------------
+// `id` is the cell on the minus side of the face.
+template <typename T, int D>
+__device__ __forceinline__ void face_flux(const Layout& L, const T* __restrict__ P, const T* __restrict__ met,
+                                          long long id, const Par<T>& par, T* Phi) {
+  const long long s = L.stride(D);
+  T qL[NV], qR[NV];
+#pragma unroll
+  for (int q = 0; q < NV; q++) {
+    const T* a = P + q * L.fs + id;
+    const T qm = a[-s], q0 = a[0], q1 = a[s], q2 = a[2 * s];
+    qL[q] = q0 + T(0.5) * mc_slope(qm, q0, q1);
+    qR[q] = q1 - T(0.5) * mc_slope(q0, q1, q2);
+  }
+  T mf[NM];
+#pragma unroll
+  for (int c = 0; c < NM; c++) mf[c] = T(0.5) * (met[c * L.fs + id] + met[c * L.fs + id + s]);
+  hlle_face<T, D>(qL, qR, mf, par, Phi);
+}
+
+template <typename T, int D>
+__device__ __forceinline__ void flux_difference(const Layout& L, const T* __restrict__ P, const T* __restrict__ met,
+                                                long long id, const Par<T>& par, T* R) {
+  T Pp[NV], Pm[NV];
+  face_flux<T, D>(L, P, met, id, par, Pp);
+  face_flux<T, D>(L, P, met, id - L.stride(D), par, Pm);
+  const T ih = T(1.0 / L.h[D]);
+#pragma unroll
+  for (int q = 0; q < NV; q++) R[q] -= (Pp[q] - Pm[q]) * ih;
+}
+
+// ---- a6: metric derivatives, fluid and cleaning sources at a cell ---------------------------------
+template <typename T>
+__device__ __forceinline__ void add_sources(const Layout& L, const T* __restrict__ met, long long id, const T* q,
+                                            const Par<T>& par, T* R) {
+  T m[NM];
+  load_fields(met, L.fs, id, NM, m);
+  T c[6], gi[6];
+  const T det = cofactors(m + GXX, c);
+  const T sq = sqrt_(det);
+  const T idet = rcp_(det);
+#pragma unroll
+  for (int a = 0; a < 6; a++) gi[a] = c[a] * idet;
+  T dm[3][NM];
+  T dQ[3] = {0, 0, 0};  // sum_j d_j(alpha sqrt(gamma) gamma^{kj})
+  T dRb = 0;            // sum_j d_j(sqrt(gamma) beta^j)
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    if (L.g[d] == 0) {
+#pragma unroll
+      for (int a = 0; a < NM; a++) dm[d][a] = 0;
+      continue;
+    }
+    const long long s = L.stride(d);
+    const T i2h = T(1.0 / (2 * L.h[d]));
+    T mp[NM], mm[NM];
+    load_fields(met, L.fs, id + s, NM, mp);
+    load_fields(met, L.fs, id - s, NM, mm);
+#pragma unroll
+    for (int a = 0; a < NM; a++) dm[d][a] = (mp[a] - mm[a]) * i2h;
+    if (par.cleaning) {
+      T cp[6], cm[6];
+      const T dp = cofactors(mp + GXX, cp), dn = cofactors(mm + GXX, cm);
+      const T sp = sqrt_(dp), sm = sqrt_(dn);
+      const T ap = mp[AL] / sp, am = mm[AL] / sm;  // alpha sqrt(gamma) gamma^{kd} = alpha cof_kd / sqrt(gamma)
+#pragma unroll
+      for (int k = 0; k < 3; k++) dQ[k] += (ap * cp[sym(k, d)] - am * cm[sym(k, d)]) * i2h;
+      dRb += (sp * mp[BEX + d] - sm * mm[BEX + d]) * i2h;
+    }
+  }
+  fluid_source(q, m, dm, par, gi, sq, R);
+  if (par.cleaning) {  // cleaning sources (R14), not multiplied by alpha
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+      T adv = q[BX] * dm[0][BEX + k] + q[BY] * dm[1][BEX + k] + q[BZ] * dm[2][BEX + k];
+      R[5 + k] += -sq * adv + q[PSI] * dQ[k];
+    }
+    T Bda = q[BX] * dm[0][AL] + q[BY] * dm[1][AL] + q[BZ] * dm[2][AL];
+    R[8] += sq * Bda - q[PSI] * dRb - m[AL] * par.kappa * sq * q[PSI];
+  } else {
+    R[8] = 0;
+  }
+}
+
+// ---- a1-a7: L(U) of one cell and the Runge-Kutta stage combine (O7) ---------------------
+// stage 0: Uout = Uin + dt L;  1: Uout = 3/4 U0 + 1/4 (Uin + dt L);  2: Uout = 1/3 U0 + 2/3 (Uin + dt L)
+template <typename T>
+__global__ void __launch_bounds__(BLK) k_rhs_update(Layout L, Par<T> par, const T* __restrict__ P,
+                                                    const T* __restrict__ met, const T* __restrict__ Uin,
+                                                    const T* __restrict__ U0, T* __restrict__ Uout, int stage, T dt) {
+  const long long n = L.ncell();
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  int i, j, k;
+  cell_of(L, t, i, j, k);
+  const long long id = L.idx(i, j, k);
+  T R[NV];
+#pragma unroll
+  for (int q = 0; q < NV; q++) R[q] = 0;
+  if (L.g[0]) flux_difference<T, 0>(L, P, met, id, par, R);
+  if (L.g[1]) flux_difference<T, 1>(L, P, met, id, par, R);
+  if (L.g[2]) flux_difference<T, 2>(L, P, met, id, par, R);
+  T q[NV];
+  load_fields(P, L.fs, id, NV, q);
+  add_sources(L, met, id, q, par, R);
+#pragma unroll
+  for (int v = 0; v < NV; v++) {
+    T u1 = Uin[v * L.fs + id] + dt * R[v];
+    if (stage == 1) u1 = T(0.75) * U0[v * L.fs + id] + T(0.25) * u1;
+    if (stage == 2) u1 = T(1.0 / 3.0) * U0[v * L.fs + id] + T(2.0 / 3.0) * u1;
+    Uout[v * L.fs + id] = u1;
+  }
+}
+
+// ---- a8: Newton-Raphson recovery + floors; U is rewritten where a floor acted ---------------------
+// counters: [0] c2p_fail, [1] atm_reset, [2] p_floor, [3] max iterations seen
+template <typename T>
+__global__ void __launch_bounds__(BLK) k_con2prim(Layout L, Par<T> par, T* __restrict__ U, const T* __restrict__ met,
+                                                  T* __restrict__ P, unsigned long long* __restrict__ counters) {
+  const long long n = L.ncell();
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool active = t < n;
+  int fail = 0, reset = 0, pfl = 0, it = 0;
+  if (active) {
+    int i, j, k;
+    cell_of(L, t, i, j, k);
+    const long long id = L.idx(i, j, k);
+    T m[NM];
+    load_fields(met, L.fs, id, NM, m);
+    T c[6], gi[6];
+    const T det = cofactors(m + GXX, c);
+    const T sq = sqrt_(det);
+    const T idet = rcp_(det);
+#pragma unroll
+    for (int a = 0; a < 6; a++) gi[a] = c[a] * idet;
+    T w[NV];
+#pragma unroll
+    for (int v = 0; v < NV; v++) w[v] = U[v * L.fs + id] / sq;
+    if (!par.cleaning) w[8] = 0;
+    T old[NV];
+    load_fields(P, L.fs, id, NV, old);
+    T Zg;
+    {  // guess from the previous primitives of this cell
+      T utl[3];
+      lower(m + GXX, old + UX, utl);
+      T W2 = 1 + dot3(old + UX, utl);
+      Zg = old[RHO] * (1 + par.gg1 * old[PR] / old[RHO]) * W2;
+    }
+    T q[NV];
+    fail = con2prim(w, m, gi, par, Zg, q, it);
+    if (fail) reset = 1;
+    else if (q[RHO] < par.rho_thr) reset = 1;
+    if (reset) {
+      q[RHO] = par.rho_atm; q[PR] = par.p_atm;
+#pragma unroll
+      for (int a = 0; a < 3; a++) { q[UX + a] = 0; q[BX + a] = w[5 + a]; }
+      q[PSI] = w[8];
+    } else if (q[PR] < par.p_atm) {
+      pfl = 1;
+      q[PR] = par.p_atm;
+    }
+#pragma unroll
+    for (int v = 0; v < NV; v++) P[v * L.fs + id] = q[v];
+    if (reset || pfl) {
+      T u[NV];
+      prim2con(q, m, par, u);
+#pragma unroll
+      for (int v = 0; v < NV; v++) U[v * L.fs + id] = sq * u[v];
+    }
+  }
+  // warp-level reduction of the counters
+  const unsigned full = 0xffffffffu;
+  const int nf = __popc(__ballot_sync(full, fail)), nr = __popc(__ballot_sync(full, reset)),
+            np = __popc(__ballot_sync(full, pfl));
+  const int mi = __reduce_max_sync(full, it);
+  if ((threadIdx.x & 31) == 0) {
+    if (nf) atomicAdd(counters + 0, (unsigned long long)nf);
+    if (nr) atomicAdd(counters + 1, (unsigned long long)nr);
+    if (np) atomicAdd(counters + 2, (unsigned long long)np);
+    if ((unsigned long long)mi > counters[3]) atomicMax(counters + 3, (unsigned long long)mi);
+  }
+}
+
+// ---- a10: global reductions with warp shuffles ---------------------------------
+// Block partial layout: [0..8] sums of U, [9] sum |divB|, [10] max |divB|, [11] max speed/dx
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+  return v;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_diag(Layout L, Par<T> par, const T* __restrict__ P, const T* __restrict__ U,
+                                              const T* __restrict__ met, double* __restrict__ partials) {
+  const long long n = L.ncell();
+  double acc[12];
+#pragma unroll
+  for (int a = 0; a < 12; a++) acc[a] = 0;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+    int i, j, k;
+    cell_of(L, t, i, j, k);
+    const long long id = L.idx(i, j, k);
+#pragma unroll
+    for (int v = 0; v < NV; v++) acc[v] += (double)U[v * L.fs + id];
+    T m[NM], q[NV];
+    load_fields(met, L.fs, id, NM, m);
+    load_fields(P, L.fs, id, NV, q);
+    T c[6];
+    const T det = cofactors(m + GXX, c);
+    const T sq = sqrt_(det), idet = rcp_(det);
+    double div = 0, smax = 0;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+      if (L.g[d] == 0) continue;
+      const long long s = L.stride(d);
+      T gp[6], gm[6];
+#pragma unroll
+      for (int a = 0; a < 6; a++) { gp[a] = met[(GXX + a) * L.fs + id + s]; gm[a] = met[(GXX + a) * L.fs + id - s]; }
+      const double bp = (double)sqrt_det(gp) * (double)P[(BX + d) * L.fs + id + s];
+      const double bm = (double)sqrt_det(gm) * (double)P[(BX + d) * L.fs + id - s];
+      div += (bp - bm) / (2 * L.h[d]);
+      T gid[3], Uu[NV], Ff[NV], lm, lp;
+#pragma unroll
+      for (int kk = 0; kk < 3; kk++) gid[kk] = c[sym(kk, d)] * idet;
+      if (d == 0) flux_speeds<T, 0>(q, m, gid, par, Uu, Ff, lm, lp);
+      if (d == 1) flux_speeds<T, 1>(q, m, gid, par, Uu, Ff, lm, lp);
+      if (d == 2) flux_speeds<T, 2>(q, m, gid, par, Uu, Ff, lm, lp);
+      smax = fmax(smax, fmax(fabs((double)lm), fabs((double)lp)) / L.h[d]);
+    }
+    div /= (double)sq;
+    acc[9] += fabs(div);
+    acc[10] = fmax(acc[10], fabs(div));
+    acc[11] = fmax(acc[11], smax);
+  }
+  __shared__ double sh[8][12];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int a = 0; a < 12; a++) {
+    double v = a < 10 ? warp_sum(acc[a]) : warp_max(acc[a]);
+    if (lane == 0) sh[wid][a] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 12) {
+    const int a = threadIdx.x;
+    double v = sh[0][a];
+    for (int w = 1; w < 8; w++) v = a < 10 ? v + sh[w][a] : fmax(v, sh[w][a]);
+    partials[(long long)blockIdx.x * NDIAG + a] = v;
+  }
+}
+
+// one block: fold the block partials in a fixed order (deterministic result)
+__global__ void k_diag_final(const double* __restrict__ partials, int nblocks, double* __restrict__ out) {
+  const int a = threadIdx.x;
+  if (a >= 12) return;
+  double v = partials[a];
+  for (int b = 1; b < nblocks; b++) {
+    const double p = partials[(long long)b * NDIAG + a];
+    v = a < 10 ? v + p : fmax(v, p);
+  }
+  out[a] = v;
+}
+
+}  // namespace hz

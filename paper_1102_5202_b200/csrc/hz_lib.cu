@@ -1,0 +1,426 @@
+// hz_lib.cu -- the C ABI of include/hz.h: context, memory plan, host/device marshalling, launches.
+// Host logic only; all arithmetic is in hz_kernels.cuh / hz_physics.cuh.  No CPU fallback exists.
+#include "../../include/hz.h"
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "hz_kernels.cuh"
+
+using namespace hz;
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline size_t elem_size(int dtype) { return dtype == HZ_F64 ? 8 : 4; }
+
+bool grid_ok(const hz_grid* G) {
+  if (!G) return false;
+  const int n3[3] = {G->nx, G->ny, G->nz};
+  if (!(G->dx > 0) || !(G->dy > 0) || !(G->dz > 0)) return false;
+  if (!std::isfinite(G->dx) || !std::isfinite(G->dy) || !std::isfinite(G->dz)) return false;
+  for (int d = 0; d < 3; d++) {
+    if (n3[d] < 1) return false;
+    if (n3[d] > 1 && n3[d] < NG) return false;
+    if (G->bc[d] != HZ_BC_PERIODIC && G->bc[d] != HZ_BC_OUTFLOW) return false;
+  }
+  return true;
+}
+
+Layout make_layout(const hz_grid& G, int dtype) {
+  Layout L;
+  const int n3[3] = {G.nx, G.ny, G.nz};
+  const int ae = (int)(128 / elem_size(dtype));  // elements per 128 bytes
+  for (int d = 0; d < 3; d++) {
+    L.n[d] = n3[d];
+    L.g[d] = n3[d] > 1 ? NG : 0;
+    L.N[d] = L.n[d] + 2 * L.g[d];
+    L.bc[d] = G.bc[d];
+  }
+  L.h[0] = G.dx; L.h[1] = G.dy; L.h[2] = G.dz;
+  L.ox = L.g[0] ? ae : 0;  // first interior element of a row on a 128-byte boundary
+  L.pitch = (int)align_up((size_t)(L.ox + L.n[0] + L.g[0]), ae);
+  L.sz = (long long)L.pitch * L.N[1];
+  L.fs = (long long)align_up((size_t)(L.sz * L.N[2]), ae);
+  return L;
+}
+
+// Memory plan: offsets (bytes) of every resident array inside the one device buffer.
+struct Plan {
+  size_t met, P[2], U[2], staging, partials, diag_out, counters, err, total;
+  int diag_blocks;
+};
+Plan make_plan(const Layout& L, int dtype) {
+  Plan p;
+  const size_t es = elem_size(dtype);
+  const size_t field = (size_t)L.fs * es;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
+  p.met = take(NM * field);
+  p.P[0] = take(NV * field);
+  p.P[1] = take(NV * field);
+  p.U[0] = take(NV * field);
+  p.U[1] = take(NV * field);
+  p.staging = take((size_t)NM * (size_t)L.ncell() * es);
+  long long nb = (L.ncell() + 255) / 256;
+  p.diag_blocks = (int)(nb < 1184 ? nb : 1184);  // 148 SMs x 8 resident blocks
+  p.partials = take((size_t)p.diag_blocks * NDIAG * sizeof(double));
+  p.diag_out = take(NDIAG * sizeof(double));
+  p.counters = take(4 * sizeof(unsigned long long));
+  p.err = take(sizeof(int));
+  p.total = o;
+  return p;
+}
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+}  // namespace
+
+struct hz_ctx {
+  hz_grid G;
+  hz_params par;
+  int dtype;
+  Layout L;
+  Plan plan;
+  cudaStream_t stream;
+  char* base;
+  bool own;
+  int cur;    // U[cur] holds the current conserved state
+  int u0;     // U[u0] holds the state at the start of the step (valid in stages 1, 2)
+  int pcur;   // P[pcur] holds the current primitives
+  int stage;  // next Runge-Kutta stage 0, 1, 2
+  bool have_metric, have_prim;
+  long long launches;
+
+  template <typename T> T* met() const { return (T*)(base + plan.met); }
+  template <typename T> T* P(int w) const { return (T*)(base + plan.P[w]); }
+  template <typename T> T* U(int w) const { return (T*)(base + plan.U[w]); }
+  template <typename T> T* staging() const { return (T*)(base + plan.staging); }
+  double* partials() const { return (double*)(base + plan.partials); }
+  double* diag_out() const { return (double*)(base + plan.diag_out); }
+  unsigned long long* counters() const { return (unsigned long long*)(base + plan.counters); }
+  int* err() const { return (int*)(base + plan.err); }
+};
+
+namespace {
+
+template <typename T>
+Par<T> make_par(const hz_ctx* c) {
+  Par<T> p;
+  const hz_params& h = c->par;
+  p.Gam = (T)h.gamma_ad;
+  p.gg1 = (T)(h.gamma_ad / (h.gamma_ad - 1));
+  p.g1g = (T)((h.gamma_ad - 1) / h.gamma_ad);
+  p.rho_atm = (T)h.rho_atm;
+  p.p_atm = (T)h.p_atm;
+  p.rho_thr = (T)(h.rho_atm * (1 + h.atm_tol));
+  p.kappa = (T)h.kappa;
+  p.c2p_tol = (T)(h.c2p_tol > 0 ? h.c2p_tol : (sizeof(T) == 8 ? 1e-13 : 1e-6));
+  p.c2p_maxit = h.c2p_maxit;
+  p.cleaning = h.cleaning;
+  return p;
+}
+
+inline unsigned nblocks(long long n, int b) { return (unsigned)((n + b - 1) / b); }
+
+#define HZ_CUDA(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return HZ_ECUDA; } } while (0)
+#define HZ_LAUNCHED(c) do { (c)->launches++; if (cudaGetLastError() != cudaSuccess) return HZ_ECUDA; } while (0)
+
+// Bring `count` elements at user pointer `src` (host or device) to the device; returns the device
+// pointer to read (the staging area for host sources).
+template <typename T>
+int to_device(hz_ctx* c, const void* src, size_t count, T* stage_at, const T** out) {
+  if (is_device_ptr(src)) { *out = (const T*)src; return HZ_OK; }
+  HZ_CUDA(cudaMemcpyAsync(stage_at, src, count * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+  *out = stage_at;
+  return HZ_OK;
+}
+
+int read_err(hz_ctx* c, int* flag) {
+  HZ_CUDA(cudaMemcpyAsync(flag, c->err(), sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  HZ_CUDA(cudaStreamSynchronize(c->stream));
+  return HZ_OK;
+}
+
+template <typename T>
+int set_metric_t(hz_ctx* c, const void* alpha, const void* beta3, const void* gamma6) {
+  const Layout& L = c->L;
+  const size_t n = (size_t)L.ncell();
+  const T *a, *b, *g;
+  T* st = c->staging<T>();
+  int rc;
+  if ((rc = to_device<T>(c, alpha, n, st, &a))) return rc;
+  if ((rc = to_device<T>(c, beta3, 3 * n, st + n, &b))) return rc;
+  if ((rc = to_device<T>(c, gamma6, 6 * n, st + 4 * n, &g))) return rc;
+  HZ_CUDA(cudaMemsetAsync(c->err(), 0, sizeof(int), c->stream));
+  k_pack_metric<T><<<nblocks(n, 256), 256, 0, c->stream>>>(L, a, b, g, c->met<T>(), c->err());
+  HZ_LAUNCHED(c);
+  const long long ntot = (long long)L.N[0] * L.N[1] * L.N[2];
+  k_fill_ghosts<T><<<nblocks(ntot, 256), 256, 0, c->stream>>>(L, c->met<T>(), NM);
+  HZ_LAUNCHED(c);
+  int flag = 0;
+  if ((rc = read_err(c, &flag))) return rc;
+  c->have_prim = false;
+  c->have_metric = flag == 0;
+  return flag ? HZ_EINVAL : HZ_OK;
+}
+
+template <typename T>
+int fill_ghosts_P(hz_ctx* c) {
+  const Layout& L = c->L;
+  if (!(L.g[0] | L.g[1] | L.g[2])) return HZ_OK;
+  const long long ntot = (long long)L.N[0] * L.N[1] * L.N[2];
+  k_fill_ghosts<T><<<nblocks(ntot, 256), 256, 0, c->stream>>>(L, c->P<T>(c->pcur), NV);
+  HZ_LAUNCHED(c);
+  return HZ_OK;
+}
+
+template <typename T>
+int set_prims_t(hz_ctx* c, const void* prim8) {
+  const Layout& L = c->L;
+  const size_t n = (size_t)L.ncell();
+  const T* p;
+  int rc;
+  if ((rc = to_device<T>(c, prim8, 8 * n, c->staging<T>(), &p))) return rc;
+  HZ_CUDA(cudaMemsetAsync(c->err(), 0, sizeof(int), c->stream));
+  HZ_CUDA(cudaMemsetAsync(c->counters(), 0, 4 * sizeof(unsigned long long), c->stream));
+  c->cur = 0; c->u0 = 1; c->pcur = 0; c->stage = 0;
+  k_pack_prims<T><<<nblocks(n, 128), 128, 0, c->stream>>>(L, make_par<T>(c), p, c->met<T>(), c->P<T>(0), c->U<T>(0),
+                                                          c->err());
+  HZ_LAUNCHED(c);
+  if ((rc = fill_ghosts_P<T>(c))) return rc;
+  int flag = 0;
+  if ((rc = read_err(c, &flag))) return rc;
+  c->have_prim = flag == 0;
+  return flag ? HZ_EINVAL : HZ_OK;
+}
+
+template <typename T>
+int substep_t(hz_ctx* c, double dt) {
+  const Layout& L = c->L;
+  const long long n = L.ncell();
+  const Par<T> par = make_par<T>(c);
+  const int st = c->stage;
+  const T* Uin = c->U<T>(c->cur);
+  T* Uout = st == 0 ? c->U<T>(1 - c->cur) : c->U<T>(c->cur);
+  const T* U0 = st == 0 ? Uin : c->U<T>(c->u0);
+  k_rhs_update<T><<<nblocks(n, BLK), BLK, 0, c->stream>>>(L, par, c->P<T>(c->pcur), c->met<T>(), Uin, U0, Uout, st,
+                                                          (T)dt);
+  HZ_LAUNCHED(c);
+  if (st == 0) { c->u0 = c->cur; c->cur = 1 - c->cur; }
+  k_con2prim<T><<<nblocks(n, BLK), BLK, 0, c->stream>>>(L, par, c->U<T>(c->cur), c->met<T>(), c->P<T>(c->pcur),
+                                                        c->counters());
+  HZ_LAUNCHED(c);
+  int rc;
+  if ((rc = fill_ghosts_P<T>(c))) return rc;
+  c->stage = (st + 1) % 3;
+  return HZ_OK;
+}
+
+// Run a kernel result out to the user: directly if `dst` is a device pointer, else through staging.
+template <typename T, typename Launch>
+int to_user(hz_ctx* c, void* dst, size_t count, Launch launch) {
+  const bool dev = is_device_ptr(dst);
+  T* out = dev ? (T*)dst : c->staging<T>();
+  launch(out);
+  HZ_LAUNCHED(c);
+  if (!dev) HZ_CUDA(cudaMemcpyAsync(dst, out, count * sizeof(T), cudaMemcpyDeviceToHost, c->stream));
+  HZ_CUDA(cudaStreamSynchronize(c->stream));
+  return HZ_OK;
+}
+
+template <typename T>
+int get_prims_t(hz_ctx* c, void* prim8) {
+  const Layout& L = c->L;
+  const long long n = L.ncell();
+  return to_user<T>(c, prim8, 8 * (size_t)n, [&](T* out) {
+    k_unpack_prims<T><<<nblocks(n, 256), 256, 0, c->stream>>>(L, c->P<T>(c->pcur), c->met<T>(), out);
+  });
+}
+template <typename T>
+int get_fields_t(hz_ctx* c, const T* F, int f0, int nf, void* dst) {
+  const Layout& L = c->L;
+  const long long n = L.ncell();
+  return to_user<T>(c, dst, (size_t)nf * (size_t)n, [&](T* out) {
+    k_unpack_fields<T><<<nblocks(n, 256), 256, 0, c->stream>>>(L, F, f0, nf, out);
+  });
+}
+
+template <typename T>
+int diag_t(hz_ctx* c, hz_diag* out) {
+  const Layout& L = c->L;
+  const int nb = c->plan.diag_blocks;
+  k_diag<T><<<nb, 256, 0, c->stream>>>(L, make_par<T>(c), c->P<T>(c->pcur), c->U<T>(c->cur), c->met<T>(), c->partials());
+  HZ_LAUNCHED(c);
+  k_diag_final<<<1, 32, 0, c->stream>>>(c->partials(), nb, c->diag_out());
+  HZ_LAUNCHED(c);
+  double h[12];
+  unsigned long long cnt[4];
+  HZ_CUDA(cudaMemcpyAsync(h, c->diag_out(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  HZ_CUDA(cudaMemcpyAsync(cnt, c->counters(), sizeof(cnt), cudaMemcpyDeviceToHost, c->stream));
+  HZ_CUDA(cudaStreamSynchronize(c->stream));
+  const double dV = L.h[0] * L.h[1] * L.h[2];
+  out->sumD = h[0] * dV; out->sumSx = h[1] * dV; out->sumSy = h[2] * dV; out->sumSz = h[3] * dV;
+  out->sumTau = h[4] * dV; out->sumBx = h[5] * dV; out->sumBy = h[6] * dV; out->sumBz = h[7] * dV;
+  out->sumPsi = h[8] * dV;
+  out->divB_L1 = h[9] / (double)L.ncell();
+  out->divB_max = h[10];
+  out->max_speed_over_dx = h[11];
+  out->c2p_fail = (long long)cnt[0]; out->atm_reset = (long long)cnt[1]; out->p_floor = (long long)cnt[2];
+  out->c2p_maxit_seen = (int)cnt[3];
+  return HZ_OK;
+}
+
+}  // namespace
+
+#define HZ_DISPATCH(c, fn, ...) ((c)->dtype == HZ_F64 ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
+
+extern "C" {
+
+int hz_default_params(hz_params* p) {
+  if (!p) return HZ_EINVAL;
+  p->gamma_ad = 4.0 / 3.0;
+  p->rho_atm = 1e-12; p->p_atm = 1e-14; p->atm_tol = 1e-3;
+  p->cleaning = 1; p->kappa = 1.0;
+  p->c2p_maxit = 30; p->c2p_tol = 0.0;
+  return HZ_OK;
+}
+
+int hz_state_bytes(const hz_grid* grid, int dtype, size_t* bytes) {
+  if (!grid_ok(grid) || !bytes || (dtype != HZ_F32 && dtype != HZ_F64)) return HZ_EINVAL;
+  *bytes = make_plan(make_layout(*grid, dtype), dtype).total;
+  return HZ_OK;
+}
+
+int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* device_buffer, hz_ctx** out) {
+  if (!out) return HZ_EINVAL;
+  *out = nullptr;
+  if (!grid_ok(grid) || (dtype != HZ_F32 && dtype != HZ_F64)) return HZ_EINVAL;
+  hz_params par;
+  if (params) par = *params; else hz_default_params(&par);
+  if (!(par.gamma_ad > 1) || par.c2p_maxit < 1 || !(par.rho_atm > 0) || !(par.p_atm > 0) || !(par.atm_tol >= 0))
+    return HZ_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return HZ_ECUDA; }
+  hz_ctx* c = new (std::nothrow) hz_ctx();
+  if (!c) return HZ_ENOMEM;
+  c->G = *grid; c->par = par; c->dtype = dtype;
+  c->L = make_layout(*grid, dtype);
+  c->plan = make_plan(c->L, dtype);
+  c->stream = 0;
+  c->own = device_buffer == nullptr;
+  if (c->own) {
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, c->plan.total);
+    if (e != cudaSuccess) { cudaGetLastError(); delete c; return e == cudaErrorMemoryAllocation ? HZ_ENOMEM : HZ_ECUDA; }
+    c->base = (char*)p;
+  } else {
+    if (((uintptr_t)device_buffer & 255) != 0 || !is_device_ptr(device_buffer)) { delete c; return HZ_EINVAL; }
+    c->base = (char*)device_buffer;
+  }
+  // zero everything once so padding never holds NaN patterns
+  if (cudaMemset(c->base, 0, c->plan.total) != cudaSuccess) {
+    cudaGetLastError();
+    if (c->own) cudaFree(c->base);
+    delete c;
+    return HZ_ECUDA;
+  }
+  c->cur = 0; c->u0 = 1; c->pcur = 0; c->stage = 0;
+  c->have_metric = c->have_prim = false;
+  c->launches = 0;
+  *out = c;
+  return HZ_OK;
+}
+
+int hz_destroy(hz_ctx* c) {
+  if (!c) return HZ_OK;
+  cudaStreamSynchronize(c->stream);
+  if (c->own && c->base) cudaFree(c->base);
+  delete c;
+  return HZ_OK;
+}
+
+int hz_set_stream(hz_ctx* c, void* cuda_stream) {
+  if (!c) return HZ_EINVAL;
+  HZ_CUDA(cudaStreamSynchronize(c->stream));
+  c->stream = (cudaStream_t)cuda_stream;
+  return HZ_OK;
+}
+
+int hz_set_metric(hz_ctx* c, const void* alpha, const void* beta3, const void* gamma6) {
+  if (!c || !alpha || !beta3 || !gamma6) return HZ_EINVAL;
+  return HZ_DISPATCH(c, set_metric_t, c, alpha, beta3, gamma6);
+}
+
+int hz_set_primitives(hz_ctx* c, const void* prim8) {
+  if (!c || !prim8) return HZ_EINVAL;
+  if (!c->have_metric) return HZ_ESTATE;
+  return HZ_DISPATCH(c, set_prims_t, c, prim8);
+}
+
+int hz_substeps(hz_ctx* c, double dt, int nsub) {
+  if (!c || nsub < 0 || !(dt > 0) || !std::isfinite(dt)) return HZ_EINVAL;
+  if (!c->have_metric || !c->have_prim) return HZ_ESTATE;
+  for (int s = 0; s < nsub; s++) {
+    int rc = HZ_DISPATCH(c, substep_t, c, dt);
+    if (rc) return rc;
+  }
+  return HZ_OK;
+}
+
+int hz_step(hz_ctx* c, double dt, int n) {
+  if (!c || n < 0) return HZ_EINVAL;
+  if (c->have_metric && c->have_prim && c->stage != 0) return HZ_ESTATE;
+  return hz_substeps(c, dt, 3 * n);
+}
+
+int hz_get_primitives(hz_ctx* c, void* prim8) {
+  if (!c || !prim8) return HZ_EINVAL;
+  if (!c->have_prim) return HZ_ESTATE;
+  return HZ_DISPATCH(c, get_prims_t, c, prim8);
+}
+
+int hz_get_psi(hz_ctx* c, void* psi) {
+  if (!c || !psi) return HZ_EINVAL;
+  if (!c->have_prim) return HZ_ESTATE;
+  if (c->dtype == HZ_F64) return get_fields_t<double>(c, c->P<double>(c->pcur), PSI, 1, psi);
+  return get_fields_t<float>(c, c->P<float>(c->pcur), PSI, 1, psi);
+}
+
+int hz_get_conserved(hz_ctx* c, void* cons9) {
+  if (!c || !cons9) return HZ_EINVAL;
+  if (!c->have_prim) return HZ_ESTATE;
+  if (c->dtype == HZ_F64) return get_fields_t<double>(c, c->U<double>(c->cur), 0, NV, cons9);
+  return get_fields_t<float>(c, c->U<float>(c->cur), 0, NV, cons9);
+}
+
+int hz_diagnostics(hz_ctx* c, hz_diag* out) {
+  if (!c || !out) return HZ_EINVAL;
+  if (!c->have_prim) return HZ_ESTATE;
+  return HZ_DISPATCH(c, diag_t, c, out);
+}
+
+long long hz_launch_count(const hz_ctx* c) { return c ? c->launches : 0; }
+
+const char* hz_strerror(int e) {
+  switch (e) {
+    case HZ_OK: return "ok";
+    case HZ_EINVAL: return "invalid argument or unphysical input";
+    case HZ_ENOMEM: return "out of device memory";
+    case HZ_ECUDA: return "CUDA error or no CUDA device";
+    case HZ_ESTATE: return "call out of order (metric/primitives not set, or mid-step)";
+    default: return "unknown error";
+  }
+}
+
+}  // extern "C"

@@ -1,0 +1,355 @@
+// hz_physics.cuh -- per-point device arithmetic of the GRMHD substep (sm_100a, fp64 and fp32).
+//
+// Every function restates a formula of DESIGN.md section 3 (readings O1-O8 of the paper's
+// pipeline) for one cell or one face, in registers.  Nothing here touches memory;
+// the kernels in hz_kernels.cuh decide what is staged where.  This file shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace hz {
+
+constexpr int NV = 9;   // rho|D, ut^i|S_i, p|tau, B^i, psi
+constexpr int NM = 10;  // alpha, beta^i, gamma_xx xy xz yy yz zz
+constexpr int NG = 2;   // ghost layers per active side: the MC stencil (R16)
+
+enum { RHO = 0, UX = 1, UY = 2, UZ = 3, PR = 4, BX = 5, BY = 6, BZ = 7, PSI = 8 };
+enum { AL = 0, BEX = 1, BEY = 2, BEZ = 3, GXX = 4, GXY = 5, GXZ = 6, GYY = 7, GYZ = 8, GZZ = 9 };
+
+// Run-time parameters in the arithmetic type of the kernels.
+template <typename T>
+struct Par {
+  T Gam;       // Gamma
+  T gg1;       // Gamma/(Gamma-1)
+  T g1g;       // (Gamma-1)/Gamma
+  T rho_atm, p_atm;
+  T rho_thr;   // rho_atm*(1+atm_tol)
+  T kappa;
+  T c2p_tol;
+  int c2p_maxit;
+  int cleaning;
+};
+
+// ---- scalar helpers -----------------------------------------------------------------------------
+__device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+__device__ __forceinline__ float sqrt_(float x) { return sqrtf(x); }
+__device__ __forceinline__ double rcp_(double x) { return 1.0 / x; }
+__device__ __forceinline__ float rcp_(float x) { return 1.0f / x; }
+__device__ __forceinline__ double abs_(double x) { return fabs(x); }
+__device__ __forceinline__ float abs_(float x) { return fabsf(x); }
+__device__ __forceinline__ double min_(double a, double b) { return fmin(a, b); }
+__device__ __forceinline__ float min_(float a, float b) { return fminf(a, b); }
+__device__ __forceinline__ double max_(double a, double b) { return fmax(a, b); }
+__device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
+__device__ __forceinline__ bool finite_(double x) { return isfinite(x); }
+__device__ __forceinline__ bool finite_(float x) { return isfinite(x); }
+
+// Lower an index with the symmetric 3-metric stored as g6 = (xx, xy, xz, yy, yz, zz).
+template <typename T>
+__device__ __forceinline__ void lower(const T* g6, const T* a, T* l) {
+  l[0] = g6[0] * a[0] + g6[1] * a[1] + g6[2] * a[2];
+  l[1] = g6[1] * a[0] + g6[3] * a[1] + g6[4] * a[2];
+  l[2] = g6[2] * a[0] + g6[4] * a[1] + g6[5] * a[2];
+}
+template <typename T>
+__device__ __forceinline__ T dot3(const T* a, const T* b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+
+// Cofactors of the symmetric 3-metric in the same packed order; det by the first column.
+template <typename T>
+__device__ __forceinline__ T cofactors(const T* g, T* c) {
+  c[0] = g[3] * g[5] - g[4] * g[4];
+  c[1] = g[4] * g[2] - g[1] * g[5];
+  c[2] = g[1] * g[4] - g[3] * g[2];
+  c[3] = g[0] * g[5] - g[2] * g[2];
+  c[4] = g[1] * g[2] - g[0] * g[4];
+  c[5] = g[0] * g[3] - g[1] * g[1];
+  return g[0] * c[0] + g[1] * c[1] + g[2] * c[2];
+}
+// Index of component (k, d) in the packed symmetric order.
+__host__ __device__ constexpr int sym(int k, int d) {
+  return k == d ? (k == 0 ? 0 : (k == 1 ? 3 : 5)) : (k + d == 1 ? 1 : (k + d == 2 ? 2 : 4));
+}
+// sqrt(gamma) of a packed 3-metric.
+template <typename T>
+__device__ __forceinline__ T sqrt_det(const T* g) {
+  T c[6];
+  return sqrt_(cofactors(g, c));
+}
+
+// MC-limited slope (O4): zero at extrema, else the smallest of twice
+// each one-sided difference and the centred difference, with the sign of the differences.
+template <typename T>
+__device__ __forceinline__ T mc_slope(T qm, T q0, T qp) {
+  T dm = q0 - qm, dp = qp - q0;
+  T s = min_(min_(2 * abs_(dm), 2 * abs_(dp)), abs_(dm + dp) * T(0.5));
+  s = dp > 0 ? s : -s;
+  return dm * dp <= 0 ? T(0) : s;
+}
+
+// ---- O1: everything one primitive state defines on a given metric -------------------------------
+template <typename T>
+struct State {
+  T W, iW, v[3], vl[3], v2, rhoh, Bl[3], B2, Bv, b2, pstar;
+  T D, S[3], tau;
+};
+
+// q = (rho, ut^i, p, B^i, psi); m = met10.  PAPER.md:60 (variables), :74 (w(u) algebraic).
+template <typename T>
+__device__ __forceinline__ void eval_state(const T* q, const T* m, const Par<T>& par, State<T>& s) {
+  T utl[3];
+  lower(m + GXX, q + UX, utl);
+  T ut2 = dot3(q + UX, utl);
+  s.W = sqrt_(1 + ut2);
+  s.iW = rcp_(s.W);
+#pragma unroll
+  for (int i = 0; i < 3; i++) { s.v[i] = q[UX + i] * s.iW; s.vl[i] = utl[i] * s.iW; }
+  s.v2 = ut2 * s.iW * s.iW;
+  s.rhoh = q[RHO] * (1 + par.gg1 * q[PR] / q[RHO]);
+  lower(m + GXX, q + BX, s.Bl);
+  s.B2 = dot3(q + BX, s.Bl);
+  s.Bv = dot3(q + BX, s.vl);
+  s.b2 = s.B2 * s.iW * s.iW + s.Bv * s.Bv;
+  s.pstar = q[PR] + s.b2 * T(0.5);
+  T Z = s.rhoh * s.W * s.W;
+  s.D = q[RHO] * s.W;
+#pragma unroll
+  for (int j = 0; j < 3; j++) s.S[j] = (Z + s.B2) * s.vl[j] - s.Bv * s.Bl[j];
+  s.tau = Z - q[PR] + (s.B2 * (1 + s.v2) - s.Bv * s.Bv) * T(0.5) - s.D;
+}
+
+// prim -> undensitised conserved (D, S_j, tau, B^k, psi).
+template <typename T>
+__device__ __forceinline__ void prim2con(const T* q, const T* m, const Par<T>& par, T* w) {
+  State<T> s;
+  eval_state(q, m, par, s);
+  w[0] = s.D; w[1] = s.S[0]; w[2] = s.S[1]; w[3] = s.S[2]; w[4] = s.tau;
+  w[5] = q[BX]; w[6] = q[BY]; w[7] = q[BZ]; w[8] = q[PSI];
+}
+
+// ---- O2 + O3: coordinate flux and coordinate signal speeds of one state along D ------------------
+// gid[k] = gamma^{kD} of the face metric.  PAPER.md:52-56 (eq. 2 in 3+1 variables), :78.
+template <typename T, int D>
+__device__ __forceinline__ void flux_speeds(const T* q, const T* m, const T* gid, const Par<T>& par,
+                                            T* U, T* F, T& lm, T& lp) {
+  State<T> s;
+  eval_state(q, m, par, s);
+  const T al = m[AL], be = m[BEX + D];
+  const T vt = al * s.v[D] - be;  // alpha (v^D - beta^D/alpha)
+  const T Bd = q[BX + D];
+  U[0] = s.D; U[1] = s.S[0]; U[2] = s.S[1]; U[3] = s.S[2]; U[4] = s.tau;
+  U[5] = q[BX]; U[6] = q[BY]; U[7] = q[BZ]; U[8] = q[PSI];
+  F[0] = s.D * vt;
+  const T aBd = al * Bd * s.iW;
+#pragma unroll
+  for (int j = 0; j < 3; j++) {
+    T bj = s.Bl[j] * s.iW + s.W * s.Bv * s.vl[j];
+    F[1 + j] = s.S[j] * vt - bj * aBd;
+  }
+  F[1 + D] += al * s.pstar;
+  F[4] = s.tau * vt + al * s.pstar * s.v[D] - al * s.Bv * Bd;
+  if (par.cleaning) {
+#pragma unroll
+    for (int k = 0; k < 3; k++) F[5 + k] = vt * q[BX + k] - al * s.v[k] * Bd + al * gid[k] * q[PSI];
+    F[8] = al * Bd - be * q[PSI];
+  } else {
+#pragma unroll
+    for (int k = 0; k < 3; k++) F[5 + k] = vt * q[BX + k] - (al * s.v[k] - m[BEX + k]) * Bd;
+    F[8] = 0;
+  }
+  // one fast-speed bound through the relativistic addition formula (R7)
+  T cs2 = par.Gam * q[PR] / s.rhoh;
+  T vA2 = s.b2 / (s.rhoh + s.b2);
+  T a2 = cs2 + vA2 - cs2 * vA2;
+  a2 = min_(max_(a2, T(0)), T(1));
+  T den = 1 - s.v2 * a2;
+  T disc = a2 * (1 - s.v2) * (den * gid[D] - (1 - a2) * s.v[D] * s.v[D]);
+  T sq = sqrt_(max_(disc, T(0)));
+  T aod = al / den;
+  T vd = s.v[D] * (1 - a2);
+  lp = aod * (vd + sq) - be;
+  lm = aod * (vd - sq) - be;
+  if (par.cleaning) {  // light cone of the (B^D, psi) subsystem
+    T c = al * sqrt_(gid[D]);
+    lp = max_(lp, -be + c);
+    lm = min_(lm, -be - c);
+  }
+}
+
+// ---- O5: HLLE flux through one face, Phi = sqrt(gamma_f) * Fhat --------------
+// qL, qR: reconstructed states (floored here); mf: face metric (mean of the two cells, R8).
+template <typename T, int D>
+__device__ __forceinline__ void hlle_face(T* qL, T* qR, const T* mf, const Par<T>& par, T* Phi) {
+  qL[RHO] = max_(qL[RHO], par.rho_atm); qL[PR] = max_(qL[PR], par.p_atm);
+  qR[RHO] = max_(qR[RHO], par.rho_atm); qR[PR] = max_(qR[PR], par.p_atm);
+  T c[6];
+  const T det = cofactors(mf + GXX, c);
+  const T sq = sqrt_(det);
+  const T idet = rcp_(det);
+  T gid[3];
+#pragma unroll
+  for (int k = 0; k < 3; k++) gid[k] = c[sym(k, D)] * idet;
+  T UL[NV], FL[NV], UR[NV], FR[NV], lmL, lpL, lmR, lpR;
+  flux_speeds<T, D>(qL, mf, gid, par, UL, FL, lmL, lpL);
+  flux_speeds<T, D>(qR, mf, gid, par, UR, FR, lmR, lpR);
+  const T lp = max_(T(0), max_(lpL, lpR));
+  const T lm = min_(T(0), min_(lmL, lmR));
+  const T w = lp - lm;
+  if (w > T(1e-30)) {
+    const T sw = sq / w, ll = lp * lm;
+#pragma unroll
+    for (int q = 0; q < NV; q++) Phi[q] = sw * (lp * FL[q] - lm * FR[q] + ll * (UR[q] - UL[q]));
+  } else {
+#pragma unroll
+    for (int q = 0; q < NV; q++) Phi[q] = sq * T(0.5) * (FL[q] + FR[q]);
+  }
+  if (!par.cleaning) Phi[8] = 0;
+}
+
+// ---- O6: geometric sources at a cell (eq. 2, the Gamma term) ------------------------
+// dm[j][c] = d_j met10[c] (zero rows for inactive axes).  Adds alpha*sqrt(gamma)*Sigma to R[1..4].
+template <typename T>
+__device__ __forceinline__ void fluid_source(const T* q, const T* m, const T (*dm)[NM], const Par<T>& par,
+                                             const T* gi /*6*/, T sq, T* R) {
+  State<T> s;
+  eval_state(q, m, par, s);
+  const T al = m[AL];
+  const T ial = rcp_(al), ial2 = ial * ial;
+  const T* be = m + BEX;
+  T u[4], b[4];
+  u[0] = s.W * ial;
+  b[0] = s.W * s.Bv * ial;
+#pragma unroll
+  for (int i = 0; i < 3; i++) {
+    T vti = s.v[i] - be[i] * ial;
+    u[1 + i] = s.W * vti;
+    b[1 + i] = q[BX + i] * s.iW + s.W * s.Bv * vti;
+  }
+  const T hb = s.rhoh + s.b2;
+  // T^{mu nu} = (rho h + b^2) u u + p* g^{mu nu} - b b
+  const T T00 = hb * u[0] * u[0] - s.pstar * ial2 - b[0] * b[0];
+  T T0[3], Tij[6];
+#pragma unroll
+  for (int i = 0; i < 3; i++) T0[i] = hb * u[0] * u[1 + i] + s.pstar * be[i] * ial2 - b[0] * b[1 + i];
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int k = i; k < 3; k++)
+      Tij[sym(i, k)] = hb * u[1 + i] * u[1 + k] + s.pstar * (gi[sym(i, k)] - be[i] * be[k] * ial2) - b[1 + i] * b[1 + k];
+  T bl[3];
+  lower(m + GXX, be, bl);
+  T T0l[3], gT0[3];  // T^0_i = beta_i T^{00} + gamma_ik T^{0k}
+  lower(m + GXX, T0, gT0);
+#pragma unroll
+  for (int i = 0; i < 3; i++) T0l[i] = bl[i] * T00 + gT0[i];
+  T SigS[3];
+#pragma unroll
+  for (int j = 0; j < 3; j++) {
+    const T* dg = dm[j] + GXX;
+    T w[3];
+    lower(dg, be, w);  // d_j gamma_ik beta^k
+    T bbdg = dot3(be, w);
+    T t0bdg = dot3(T0, w);
+    T t0db = dot3(T0l, dm[j] + BEX);
+    T tdg = Tij[0] * dg[0] + Tij[3] * dg[3] + Tij[5] * dg[5] + 2 * (Tij[1] * dg[1] + Tij[2] * dg[2] + Tij[4] * dg[4]);
+    SigS[j] = T00 * (bbdg * T(0.5) - al * dm[j][AL]) + t0bdg + t0db + tdg * T(0.5);
+  }
+  // T^i_j d_i beta^j with T^i_j = beta_j T^{i0} + gamma_jk T^{ik}
+  T Tdb = 0;
+#pragma unroll
+  for (int i = 0; i < 3; i++) {
+    T row[3] = {Tij[sym(i, 0)], Tij[sym(i, 1)], Tij[sym(i, 2)]};
+    T rl[3];
+    lower(m + GXX, row, rl);
+#pragma unroll
+    for (int j = 0; j < 3; j++) Tdb += (bl[j] * T0[i] + rl[j]) * dm[i][BEX + j];
+  }
+  T T0da = T0[0] * dm[0][AL] + T0[1] * dm[1][AL] + T0[2] * dm[2][AL];
+  T SigTau = (dot3(be, SigS) + Tdb) * ial - T0da;
+  const T f = al * sq;
+  R[1] += f * SigS[0]; R[2] += f * SigS[1]; R[3] += f * SigS[2];
+  R[4] += f * SigTau;
+}
+
+// ---- O8: primitive recovery, Newton-Raphson on Z = rho h W^2 (R10, R11) -------
+template <typename T>
+struct C2P { T D, S2, B2, SB, E; };
+
+template <typename T>
+__device__ __forceinline__ void c2p_eval(T Z, const C2P<T>& c, const Par<T>& par, T& v2, T& f, T& df) {
+  const T ZB = Z + c.B2;
+  const T SB2 = c.SB * c.SB;
+  const T Z2 = Z * Z;
+  const T iZ = rcp_(Z), iZB = rcp_(ZB);
+  const T iZ2 = iZ * iZ, iZB2 = iZB * iZB;
+  v2 = (c.S2 * Z2 + SB2 * (c.B2 + 2 * Z)) * iZ2 * iZB2;
+  const T omv = 1 - v2;
+  const T sq = sqrt_(omv);
+  const T p = par.g1g * (Z * omv - c.D * sq);
+  f = Z - p + c.B2 * (1 + v2) * T(0.5) - SB2 * T(0.5) * iZ2 - c.E;
+  const T dv2 = -2 * (c.S2 * Z2 * Z + SB2 * (3 * Z2 + 3 * Z * c.B2 + c.B2 * c.B2)) * (iZ2 * iZ) * (iZB2 * iZB);
+  df = 1 - par.g1g * omv - par.g1g * (-Z + c.D / (2 * sq)) * dv2 + c.B2 * dv2 * T(0.5) + SB2 * iZ2 * iZ;
+}
+
+// w: undensitised conserved; gi: inverse 3-metric (packed); Zg: guess.  Returns 0 on success.
+template <typename T>
+__device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters) {
+  C2P<T> c;
+  T Su[3], Bl[3];
+  lower(gi, w + 1, Su);
+  lower(m + GXX, w + 5, Bl);
+  c.D = w[0];
+  c.S2 = dot3(w + 1, Su);
+  c.B2 = dot3(w + 5, Bl);
+  c.SB = dot3(w + 1, w + 5);
+  c.E = w[4] + w[0];
+  iters = 0;
+  if (!(c.D > 0) || !finite_(c.D) || !finite_(c.S2) || !finite_(c.E) || !finite_(c.B2)) return 1;
+  T Z = Zg;
+  if (!(Z > 0) || !finite_(Z)) Z = c.E + c.D;
+  if (!(Z > 0)) Z = c.D;
+  T v2, f, df;
+  // move into the region v^2(Z) < 1 (v^2 falls monotonically with Z)
+  for (int k = 0; k < 200; k++) {
+    c2p_eval(Z, c, par, v2, f, df);
+    if (v2 < 1 && finite_(f)) break;
+    Z = 2 * Z;
+  }
+  if (!(v2 < 1)) return 1;
+  bool ok = false;
+  for (int it = 1; it <= par.c2p_maxit; it++) {
+    iters = it;
+    T Zn = Z - f / df;
+    T v2n, fn, dfn;
+    int halv = 0;
+    for (;;) {  // keep Z > 0 and v^2 < 1 by halving the step
+      bool good = finite_(Zn) && Zn > 0;
+      if (good) {
+        c2p_eval(Zn, c, par, v2n, fn, dfn);
+        good = v2n < 1 && finite_(fn) && finite_(dfn);
+      }
+      if (good) break;
+      if (++halv > 40) return 1;
+      Zn = (Z + Zn) * T(0.5);
+    }
+    T dZ = abs_(Zn - Z);
+    Z = Zn; v2 = v2n; f = fn; df = dfn;
+    if (dZ <= par.c2p_tol * Z) { ok = true; break; }
+  }
+  if (!ok) return 1;
+  const T omv = 1 - v2;
+  const T sq = sqrt_(omv);
+  const T W = rcp_(sq);
+  q[RHO] = c.D * sq;
+  q[PR] = par.g1g * (Z * omv - c.D * sq);
+  const T iZB = rcp_(Z + c.B2);
+  const T sbz = c.SB / Z * iZB;
+#pragma unroll
+  for (int i = 0; i < 3; i++) {
+    q[UX + i] = W * (Su[i] * iZB + sbz * w[5 + i]);
+    q[BX + i] = w[5 + i];
+  }
+  q[PSI] = w[8];
+  if (!finite_(q[RHO]) || !finite_(q[PR]) || !finite_(W)) return 1;
+  return 0;
+}
+
+}  // namespace hz
