@@ -127,6 +127,16 @@ int hz_diagnostics(hz_ctx* ctx, hz_diag* out);
 /* Number of kernels this context has launched since hz_create (bench.py's gpu_launches). */
 long long hz_launch_count(const hz_ctx* ctx);
 
+/* Per-kernel device timing of the substep kernels, for the roofline report (PAPER.md:190-194 times
+ * the main loop only).  hz_profile(ctx, 1) brackets every later substep kernel launch with CUDA
+ * events on the context stream; hz_profile_read synchronises, adds up the elapsed milliseconds and
+ * the launch counts per kernel kind (arrays of HZ_NKERNELS entries, kind k named hz_kernel_name(k))
+ * and clears the record.  At most 16384 launches are kept between reads; later ones are not timed. */
+enum { HZ_NKERNELS = 4 };
+int hz_profile(hz_ctx* ctx, int enable);
+int hz_profile_read(hz_ctx* ctx, double* ms, long long* launches);
+const char* hz_kernel_name(int kind);
+
 const char* hz_strerror(int code);
 
 #ifdef __cplusplus

@@ -12,7 +12,9 @@ HZ_OK, HZ_EINVAL, HZ_ENOMEM, HZ_ECUDA, HZ_ESTATE = 0, -1, -2, -3, -4
 # every symbol include/hz.h declares (tests check the library exports each of them)
 SYMBOLS = ["hz_default_params", "hz_state_bytes", "hz_create", "hz_destroy", "hz_set_stream", "hz_set_metric",
            "hz_set_primitives", "hz_step", "hz_substeps", "hz_get_primitives", "hz_get_psi", "hz_get_conserved",
-           "hz_diagnostics", "hz_launch_count", "hz_strerror"]
+           "hz_diagnostics", "hz_launch_count", "hz_profile", "hz_profile_read", "hz_kernel_name",
+           "hz_strerror"]
+HZ_NKERNELS = 4
 
 
 class HzGrid(C.Structure):
@@ -88,6 +90,10 @@ def lib():
         L.hz_diagnostics.argtypes = [vp, C.POINTER(HzDiag)]
         L.hz_launch_count.argtypes = [vp]
         L.hz_launch_count.restype = C.c_longlong
+        L.hz_profile.argtypes = [vp, ip]
+        L.hz_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.hz_kernel_name.argtypes = [ip]
+        L.hz_kernel_name.restype = C.c_char_p
         L.hz_strerror.argtypes = [ip]
         L.hz_strerror.restype = C.c_char_p
         _lib = L
@@ -221,6 +227,16 @@ class Horizon:
 
     def launch_count(self):
         return lib().hz_launch_count(self._h)
+
+    def profile(self, enable=True):
+        _chk(lib().hz_profile(self._h, int(bool(enable))), "hz_profile")
+
+    def profile_read(self):
+        """{kernel name: (total ms, launches)} since the last read; synchronises."""
+        ms = (C.c_double * HZ_NKERNELS)()
+        cnt = (C.c_longlong * HZ_NKERNELS)()
+        _chk(lib().hz_profile_read(self._h, ms, cnt), "hz_profile_read")
+        return {lib().hz_kernel_name(k).decode(): (ms[k], cnt[k]) for k in range(HZ_NKERNELS)}
 
     @classmethod
     def from_workload(cls, w, dtype="f64", **kw):

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "hz_kernels.cuh"
 
@@ -101,6 +102,9 @@ struct hz_ctx {
   int stage;  // next Runge-Kutta stage 0, 1, 2
   bool have_metric, have_prim;
   long long launches;
+  bool prof;                          // per-kernel event timing on (hz_profile)
+  std::vector<cudaEvent_t> ev_pool;   // pairs: [2i] start, [2i+1] stop
+  std::vector<int> ev_kind;           // kind of each recorded pair
 
   template <typename T> T* met() const { return (T*)(base + plan.met); }
   template <typename T> T* P(int w) const { return (T*)(base + plan.P[w]); }
@@ -130,6 +134,28 @@ Par<T> make_par(const hz_ctx* c) {
   p.cleaning = h.cleaning;
   return p;
 }
+
+enum { K_RHS = 0, K_C2P = 1, K_GHOST = 2, K_OTHER = 3 };
+constexpr size_t PROF_MAX = 16384;
+
+// Brackets one launch with events when profiling is on.
+struct ProfScope {
+  hz_ctx* c;
+  cudaEvent_t stop;
+  ProfScope(hz_ctx* c_, int kind) : c(c_), stop(nullptr) {
+    if (!c->prof || c->ev_kind.size() >= PROF_MAX) return;
+    const size_t i = c->ev_kind.size();
+    while (c->ev_pool.size() < 2 * (i + 1)) {
+      cudaEvent_t e;
+      if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return; }
+      c->ev_pool.push_back(e);
+    }
+    cudaEventRecord(c->ev_pool[2 * i], c->stream);
+    stop = c->ev_pool[2 * i + 1];
+    c->ev_kind.push_back(kind);
+  }
+  ~ProfScope() { if (stop) cudaEventRecord(stop, c->stream); }
+};
 
 inline unsigned nblocks(long long n, int b) { return (unsigned)((n + b - 1) / b); }
 
@@ -180,7 +206,10 @@ int fill_ghosts_P(hz_ctx* c) {
   const Layout& L = c->L;
   if (!(L.g[0] | L.g[1] | L.g[2])) return HZ_OK;
   const long long ntot = (long long)L.N[0] * L.N[1] * L.N[2];
-  k_fill_ghosts<T><<<nblocks(ntot, 256), 256, 0, c->stream>>>(L, c->P<T>(c->pcur), NV);
+  {
+    ProfScope ps(c, K_GHOST);
+    k_fill_ghosts<T><<<nblocks(ntot, 256), 256, 0, c->stream>>>(L, c->P<T>(c->pcur), NV);
+  }
   HZ_LAUNCHED(c);
   return HZ_OK;
 }
@@ -214,12 +243,18 @@ int substep_t(hz_ctx* c, double dt) {
   const T* Uin = c->U<T>(c->cur);
   T* Uout = st == 0 ? c->U<T>(1 - c->cur) : c->U<T>(c->cur);
   const T* U0 = st == 0 ? Uin : c->U<T>(c->u0);
-  k_rhs_update<T><<<nblocks(n, BLK), BLK, 0, c->stream>>>(L, par, c->P<T>(c->pcur), c->met<T>(), Uin, U0, Uout, st,
-                                                          (T)dt);
+  {
+    ProfScope ps(c, K_RHS);
+    k_rhs_update<T><<<nblocks(n, BLK), BLK, 0, c->stream>>>(L, par, c->P<T>(c->pcur), c->met<T>(), Uin, U0, Uout, st,
+                                                            (T)dt);
+  }
   HZ_LAUNCHED(c);
   if (st == 0) { c->u0 = c->cur; c->cur = 1 - c->cur; }
-  k_con2prim<T><<<nblocks(n, BLK), BLK, 0, c->stream>>>(L, par, c->U<T>(c->cur), c->met<T>(), c->P<T>(c->pcur),
-                                                        c->counters());
+  {
+    ProfScope ps(c, K_C2P);
+    k_con2prim<T><<<nblocks(n, BLK), BLK, 0, c->stream>>>(L, par, c->U<T>(c->cur), c->met<T>(), c->P<T>(c->pcur),
+                                                          c->counters());
+  }
   HZ_LAUNCHED(c);
   int rc;
   if ((rc = fill_ghosts_P<T>(c))) return rc;
@@ -338,6 +373,7 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
   c->cur = 0; c->u0 = 1; c->pcur = 0; c->stage = 0;
   c->have_metric = c->have_prim = false;
   c->launches = 0;
+  c->prof = false;
   *out = c;
   return HZ_OK;
 }
@@ -345,6 +381,7 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
 int hz_destroy(hz_ctx* c) {
   if (!c) return HZ_OK;
   cudaStreamSynchronize(c->stream);
+  for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
   if (c->own && c->base) cudaFree(c->base);
   delete c;
   return HZ_OK;
@@ -411,6 +448,38 @@ int hz_diagnostics(hz_ctx* c, hz_diag* out) {
 }
 
 long long hz_launch_count(const hz_ctx* c) { return c ? c->launches : 0; }
+
+int hz_profile(hz_ctx* c, int enable) {
+  if (!c) return HZ_EINVAL;
+  HZ_CUDA(cudaStreamSynchronize(c->stream));
+  c->prof = enable != 0;
+  c->ev_kind.clear();
+  return HZ_OK;
+}
+
+int hz_profile_read(hz_ctx* c, double* ms, long long* launches) {
+  if (!c || !ms || !launches) return HZ_EINVAL;
+  HZ_CUDA(cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < HZ_NKERNELS; k++) { ms[k] = 0; launches[k] = 0; }
+  for (size_t i = 0; i < c->ev_kind.size(); i++) {
+    float t = 0;
+    HZ_CUDA(cudaEventElapsedTime(&t, c->ev_pool[2 * i], c->ev_pool[2 * i + 1]));
+    ms[c->ev_kind[i]] += t;
+    launches[c->ev_kind[i]]++;
+  }
+  c->ev_kind.clear();
+  return HZ_OK;
+}
+
+const char* hz_kernel_name(int kind) {
+  switch (kind) {
+    case K_RHS: return "k_rhs_update";
+    case K_C2P: return "k_con2prim";
+    case K_GHOST: return "k_fill_ghosts";
+    case K_OTHER: return "other";
+    default: return "?";
+  }
+}
 
 const char* hz_strerror(int e) {
   switch (e) {

@@ -1,0 +1,277 @@
+"""GPU-vs-oracle parity through the C-ABI (pytest -m gpu).  Tolerances are BASELINE.json's north_star:
+fp64 rel. L1 <= 1e-10 per field after one substep and <= 1e-7 after the full run; fp32 <= 1e-4 after one
+substep against the fp64 oracle.  Inputs come from workloads/ (seeded, synthetic); expected values come
+from oracle/ only."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import workloads as wl
+from parity import assert_parity, oracle_for, rel_l1
+
+pytestmark = pytest.mark.gpu
+
+TOL64_SUB, TOL64_RUN, TOL32_SUB = 1e-10, 1e-7, 1e-4
+
+
+def horizon(w, dtype="f64", **kw):
+    from paper_1102_5202_b200 import Horizon
+    return Horizon.from_workload(w, dtype=dtype, **kw)
+
+
+def sub_block(w, sl):
+    """The workload restricted to the index block sl = (kslice, jslice, islice)."""
+    f = lambda a: np.ascontiguousarray(a[(slice(None),) + sl]) if a.ndim == 4 else np.ascontiguousarray(a[sl])
+    n = tuple(s.stop - s.start for s in sl[::-1])
+    return dataclasses.replace(w, n=n, alpha=f(w.alpha), beta3=f(w.beta3), gamma6=f(w.gamma6), prim8=f(w.prim8))
+
+
+# sizes span several thread blocks / tiles and leave ragged tails in every axis
+SMALL = {
+    "tube_x": lambda: wl.shock_tube(400, axis=0),
+    "tube_x_ragged": lambda: wl.shock_tube(403, axis=0),
+    "tube_y": lambda: wl.shock_tube(131, axis=1),
+    "tube_z": lambda: wl.shock_tube(77, axis=2),
+    "alfven_3d": lambda: wl.alfven_wave(n=(37, 21, 13)),
+    "alfven_2d": lambda: wl.alfven_wave(n=(45, 19, 1)),
+    "alfven_1d": lambda: wl.alfven_wave(64, direction="x"),
+    "blast": lambda: wl.blast(35),
+    "tov": lambda: wl.tov_star(44),
+    "kerr": lambda: wl.kerr_sweep(41),
+}
+
+
+@pytest.mark.parametrize("name", sorted(SMALL))
+@pytest.mark.parametrize("nsub", [1, 3])
+def test_substep_parity_fp64(name, nsub):
+    w = SMALL[name]()
+    o = oracle_for(w)
+    hz = horizon(w, "f64")
+    o.substeps(w.dt, nsub)
+    hz.substeps(w.dt, nsub)
+    assert_parity(hz.get_primitives(), o.get_primitives(), TOL64_SUB, f"{name} fp64 {nsub} substeps")
+    # cleaning scalar and densitised conserved variables too
+    psi_o, psi_g = o.get_psi(), hz.get_psi()
+    assert np.abs(psi_g - psi_o).sum() <= TOL64_SUB * max(np.abs(psi_o).sum(), 1e-300) + 1e-25
+    Uo, Ug = o.get_conserved(), hz.get_conserved()
+    for q in range(9):
+        den = np.abs(Uo[q]).sum()
+        scale = den if den > 0 else np.abs(Uo).max() * Uo[q].size
+        assert np.abs(Ug[q] - Uo[q]).sum() <= TOL64_SUB * scale, (name, q)
+    hz.close()
+
+
+@pytest.mark.parametrize("name", sorted(SMALL))
+def test_substep_parity_fp32(name):
+    w = SMALL[name]()
+    o = oracle_for(w)
+    hz = horizon(w, "f32")
+    o.substeps(w.dt, 1)
+    hz.substeps(w.dt, 1)
+    got = hz.get_primitives()
+    assert got.dtype == np.float32
+    assert_parity(got, o.get_primitives(), TOL32_SUB, f"{name} fp32 1 substep")
+    hz.close()
+
+
+def test_full_run_config1_tube_fp64():
+    """BASELINE config 1 exactly: 400 cells, CFL 0.4, 400 steps to t = 0.4."""
+    w = wl.shock_tube(400)
+    assert w.nsteps == 400
+    o = oracle_for(w)
+    hz = horizon(w, "f64")
+    o.step(w.dt, w.nsteps)
+    hz.step(w.dt, w.nsteps)
+    r = assert_parity(hz.get_primitives(), o.get_primitives(), TOL64_RUN, "tube full run")
+    assert max(r.values()) < 1e-9  # in practice round-off level
+    do, dg = o.diagnostics(), hz.diagnostics()
+    for k in ("c2p_fail", "atm_reset", "p_floor"):
+        assert do[k] == dg[k] == 0
+    hz.close()
+
+
+@pytest.mark.parametrize("name,make,nsteps", [
+    ("alfven32", lambda: wl.alfven_wave(32), None),          # config 2 at its smallest grid, one period
+    ("blast40", lambda: wl.blast(40), 20),                   # config 3 shape, 60 substeps
+    ("tov48", lambda: wl.tov_star(48), 12),                  # config 4 shape, 36 substeps
+    ("kerr40", lambda: wl.kerr_sweep(40), 34),               # config 5 shape, its full 102 substeps
+])
+def test_full_run_parity_fp64(name, make, nsteps):
+    w = make()
+    nsteps = nsteps or w.nsteps
+    o = oracle_for(w)
+    hz = horizon(w, "f64")
+    o.step(w.dt, nsteps)
+    hz.step(w.dt, nsteps)
+    assert_parity(hz.get_primitives(), o.get_primitives(), TOL64_RUN, f"{name} {nsteps} steps")
+    do, dg = o.diagnostics(), hz.diagnostics()
+    for k in ("c2p_fail", "atm_reset", "p_floor", "c2p_maxit_seen"):
+        assert do[k] == dg[k], (k, do[k], dg[k])
+    hz.close()
+
+
+def test_diagnostics_match_oracle():
+    w = wl.kerr_sweep(33)
+    o = oracle_for(w)
+    hz = horizon(w, "f64")
+    o.substeps(w.dt, 2)
+    hz.substeps(w.dt, 2)
+    do, dg = o.diagnostics(), hz.diagnostics()
+    for k in ("sumD", "sumSx", "sumSy", "sumSz", "sumTau", "sumBx", "sumBy", "sumBz", "divB_L1"):
+        assert abs(dg[k] - do[k]) <= 1e-12 * max(abs(do[k]), 1e-3), (k, dg[k], do[k])  # summation order (R21)
+    for k in ("divB_max", "max_speed_over_dx"):
+        assert abs(dg[k] - do[k]) <= 1e-11 * abs(do[k]), (k, dg[k], do[k])
+    hz.close()
+
+
+def test_bench_configuration_sampled_block_256():
+    """BASELINE config 5 at the bench size (256^3, fp64, the launch configuration bench.py times):
+    after one full RK3 step a cell depends only on cells within 3 x 3 zones of it (two for the MC
+    stencil, one for the source differences, per substep), so the oracle run on a 44^3 sub-block of the
+    same inputs fixes the inner 20^3 cells one by one."""
+    w = wl.kerr_sweep(256)
+    hz = horizon(w, "f64")
+    hz.step(w.dt, 1)
+    got = hz.get_primitives()
+    assert np.isfinite(got).all()
+    m = 12
+    for (k0, j0, i0) in [(0, 0, 0), (106, 117, 90), (212, 212, 212), (31, 200, 140)]:
+        sl = (slice(k0, k0 + 44), slice(j0, j0 + 44), slice(i0, i0 + 44))
+        ws = sub_block(w, sl)
+        o = oracle_for(ws)
+        o.step(w.dt, 1)
+        ref = o.get_primitives()
+        lo = [0 if s.start == 0 else m for s in sl]          # a true domain boundary needs no margin
+        inner = tuple(slice(a, 44 - m) for a in lo)
+        g = got[(slice(None),) + sl][(slice(None),) + inner]
+        assert_parity(g, ref[(slice(None),) + inner], TOL64_SUB * 10, f"256^3 block at {(k0, j0, i0)}")
+    hz.close()
+
+
+def test_device_pointers_and_user_buffer_agree_with_host_path():
+    import torch
+    from paper_1102_5202_b200 import Horizon, HzParams
+    w = wl.kerr_sweep(24)
+    a = horizon(w, "f64")                       # host numpy inputs, torch-owned state buffer
+    par = HzParams.default(**w.params)
+    b = Horizon(w.n, w.h, w.bc, dtype="f64", params=par, use_torch_memory=False)  # cudaMalloc'd state
+    dev = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    b.set_metric(dev(w.alpha), dev(w.beta3), dev(w.gamma6))
+    b.set_primitives(dev(w.prim8))
+    s = torch.cuda.Stream()
+    b.set_stream(s)
+    a.step(w.dt, 1)
+    b.step(w.dt, 1)
+    out = torch.empty((8,) + w.alpha.shape, dtype=torch.float64, device="cuda")
+    b.get_primitives(out=out)
+    assert np.array_equal(a.get_primitives(), out.cpu().numpy())  # deterministic per cell: bitwise equal
+    a.close(); b.close()
+
+
+def test_bitwise_reproducible():
+    w = wl.blast(32)
+    outs = []
+    for _ in range(2):
+        hz = horizon(w, "f32")
+        hz.step(w.dt, 2)
+        outs.append(hz.get_primitives())
+        hz.close()
+    assert np.array_equal(outs[0], outs[1])
+
+
+def test_uniform_state_on_constant_curved_metric_is_a_fixed_point():
+    n = (20, 12, 9)
+    alpha, beta3, gamma6 = wl.constant_metric(n)
+    prim = np.zeros((8, n[2], n[1], n[0]))
+    prim[0], prim[4] = 1.0, 0.3
+    prim[1], prim[2], prim[3] = 0.2, -0.1, 0.05
+    prim[5], prim[6], prim[7] = 0.3, 0.1, -0.2
+    from paper_1102_5202_b200 import Horizon, HzParams
+    hz = Horizon(n, (0.1, 0.1, 0.1), (0, 0, 0), params=HzParams.default(gamma_ad=5.0 / 3.0))
+    hz.set_metric(alpha, beta3, gamma6)
+    hz.set_primitives(prim)
+    hz.step(0.02, 5)
+    out = hz.get_primitives()
+    assert np.abs(out - prim).max() < 1e-13
+    hz.close()
+
+
+def test_minimum_extent_and_two_cell_axes():
+    # 2 cells along y and z (the smallest active extent), ragged x
+    w = wl.alfven_wave(n=(19, 2, 2))
+    o = oracle_for(w)
+    hz = horizon(w)
+    o.substeps(w.dt, 3)
+    hz.substeps(w.dt, 3)
+    assert_parity(hz.get_primitives(), o.get_primitives(), TOL64_SUB, "19x2x2")
+    hz.close()
+    # a single cell: nothing to sweep, the state must not change
+    from paper_1102_5202_b200 import Horizon
+    hz = Horizon((1, 1, 1), (1, 1, 1), (0, 0, 0))
+    a, b, g = wl.minkowski((1, 1, 1))
+    hz.set_metric(a, b, g)
+    p = np.array([1.0, 0.1, 0.2, -0.3, 2.0, 0.5, 0.1, 0.2]).reshape(8, 1, 1, 1)
+    hz.set_primitives(p)
+    hz.step(0.1, 2)
+    assert np.abs(hz.get_primitives() - p).max() < 1e-14
+    hz.close()
+
+
+def test_failed_recovery_resets_to_atmosphere_like_the_oracle():
+    """Degenerate case of the method: a state that evacuates a cell ends in the atmosphere branch."""
+    w = wl.blast(24)
+    w.prim8[0] = np.where(w.prim8[0] < 5e-3, 1.0000005e-7, w.prim8[0])  # ambient medium right at the floor
+    o = oracle_for(w)
+    hz = horizon(w)
+    o.step(w.dt, 3)
+    hz.step(w.dt, 3)
+    do, dg = o.diagnostics(), hz.diagnostics()
+    assert do["atm_reset"] > 0
+    assert dg["atm_reset"] == do["atm_reset"] and dg["c2p_fail"] == do["c2p_fail"] and dg["p_floor"] == do["p_floor"]
+    assert_parity(hz.get_primitives(), o.get_primitives(), TOL64_RUN, "floored blast")
+    hz.close()
+
+
+def test_errors_and_call_order():
+    from paper_1102_5202_b200 import Horizon, HzError
+    from paper_1102_5202_b200.binding import HZ_EINVAL, HZ_ESTATE
+    n = (8, 8, 8)
+    a, b, g = wl.minkowski(n)
+    p = np.zeros((8, 8, 8, 8))
+    p[0], p[4] = 1.0, 1.0
+    hz = Horizon(n, (1, 1, 1), (1, 1, 1))
+    with pytest.raises(HzError) as e:
+        hz.set_primitives(p)           # before the metric
+    assert e.value.code == HZ_ESTATE
+    with pytest.raises(HzError) as e:
+        hz.step(0.1, 1)
+    assert e.value.code == HZ_ESTATE
+    bad = g.copy(); bad[0, 3, 3, 3] = -1.0
+    with pytest.raises(HzError) as e:
+        hz.set_metric(a, b, bad)       # not positive definite
+    assert e.value.code == HZ_EINVAL
+    bad_a = a.copy(); bad_a[1, 1, 1] = np.nan
+    with pytest.raises(HzError):
+        hz.set_metric(bad_a, b, g)
+    hz.set_metric(a, b, g)
+    for f, val in ((0, 0.0), (0, -1.0), (4, -1e-3), (1, 1.0), (5, np.inf), (2, np.nan)):
+        q = p.copy(); q[f, 2, 3, 4] = val
+        with pytest.raises(HzError) as e:
+            hz.set_primitives(q)
+        assert e.value.code == HZ_EINVAL, (f, val)
+        with pytest.raises(HzError):
+            hz.step(0.1, 1)            # still no valid primitives
+    hz.set_primitives(p)
+    with pytest.raises(HzError):
+        hz.step(-0.1, 1)
+    hz.substeps(0.1, 1)
+    with pytest.raises(HzError) as e:
+        hz.step(0.1, 1)                # in the middle of a step
+    assert e.value.code == HZ_ESTATE
+    hz.substeps(0.1, 2)
+    hz.step(0.1, 1)
+    assert np.abs(hz.get_primitives() - p).max() < 1e-14
+    with pytest.raises(ValueError):
+        hz.set_primitives(p[:, :4])
+    hz.close()
