@@ -37,7 +37,29 @@ def oracle_for(w, **par_over):
     return o
 
 
-def assert_parity(gpu, ora, tol, what=""):
+def floor_flip_mask(gpu, ora, rho_atm, atm_tol, band=1e-4):
+    """Cells where exactly one side took the atmosphere-reset branch (fp32 only).
+
+    The reset `rho < rho_atm (1 + atm_tol)` is the one discontinuous decision of the scheme.  In fp32 the
+    recovered density carries an error of a few 1e-6 relative in near-vacuum cells next to dense ones,
+    so a cell whose density lands within that of the threshold may take the other branch.  Such a cell
+    is a valid result of the method, not a unique one: it is taken out of the L1 sums, but only if the
+    side that was NOT reset has its density within `band` (relative) of the threshold; the caller bounds
+    how many there may be."""
+    gpu = np.asarray(gpu, dtype=np.float64)
+    ora = np.asarray(ora, dtype=np.float64)
+    thr = rho_atm * (1 + atm_tol)
+    is_atm = lambda a: (np.abs(a[0] - rho_atm) <= 1e-6 * rho_atm) & (a[1] == 0) & (a[2] == 0) & (a[3] == 0)
+    ga, oa = is_atm(gpu), is_atm(ora)
+    flip = ga ^ oa
+    other = np.where(ga, ora[0], gpu[0])
+    return flip & (np.abs(other - thr) <= band * thr)
+
+
+def assert_parity(gpu, ora, tol, what="", mask=None):
+    if mask is not None:
+        gpu = np.where(mask[None], 0.0, np.asarray(gpu, dtype=np.float64))
+        ora = np.where(mask[None], 0.0, np.asarray(ora, dtype=np.float64))
     r = rel_l1(gpu, ora)
     bad = {k: v for k, v in r.items() if not (v <= tol)}
     assert not bad, f"{what}: rel L1 above {tol:g}: {bad} (all: {r})"
