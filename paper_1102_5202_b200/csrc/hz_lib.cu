@@ -5,11 +5,12 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
 
-#include "hz_kernels.cuh"
+#include "hz_substep.cuh"
 
 using namespace hz;
 
@@ -101,6 +102,7 @@ struct hz_ctx {
   int pcur;   // P[pcur] holds the current primitives
   int stage;  // next Runge-Kutta stage 0, 1, 2
   bool have_metric, have_prim;
+  bool unfused;  // HZ_UNFUSED=1 in the environment at hz_create: the first, three-kernel path (A/B timing only)
   long long launches;
   bool prof;                          // per-kernel event timing on (hz_profile)
   std::vector<cudaEvent_t> ev_pool;   // pairs: [2i] start, [2i+1] stop
@@ -135,7 +137,7 @@ Par<T> make_par(const hz_ctx* c) {
   return p;
 }
 
-enum { K_RHS = 0, K_C2P = 1, K_GHOST = 2, K_OTHER = 3 };
+enum { K_RHS = 0, K_C2P = 1, K_GHOST = 2, K_SUBSTEP = 3 };
 constexpr size_t PROF_MAX = 16384;
 
 // Brackets one launch with events when profiling is on.
@@ -243,6 +245,20 @@ int substep_t(hz_ctx* c, double dt) {
   const T* Uin = c->U<T>(c->cur);
   T* Uout = st == 0 ? c->U<T>(1 - c->cur) : c->U<T>(c->cur);
   const T* U0 = st == 0 ? Uin : c->U<T>(c->u0);
+  if (!c->unfused) {  // the whole substep in one kernel (hz_substep.cuh)
+    using G = TileGeom<T>;
+    const dim3 grid((L.n[0] + G::TX - 1) / G::TX, (L.n[1] + G::TY - 1) / G::TY, (L.n[2] + G::TZ - 1) / G::TZ);
+    {
+      ProfScope ps(c, K_SUBSTEP);
+      k_substep<T><<<grid, SUB_NT, G::SMEM, c->stream>>>(L, par, c->P<T>(c->pcur), c->met<T>(), Uin, U0, Uout,
+                                                          c->P<T>(1 - c->pcur), st, (T)dt, c->counters());
+    }
+    HZ_LAUNCHED(c);
+    if (st == 0) { c->u0 = c->cur; c->cur = 1 - c->cur; }
+    c->pcur = 1 - c->pcur;
+    c->stage = (st + 1) % 3;
+    return HZ_OK;
+  }
   {
     ProfScope ps(c, K_RHS);
     k_rhs_update<T><<<nblocks(n, BLK), BLK, 0, c->stream>>>(L, par, c->P<T>(c->pcur), c->met<T>(), Uin, U0, Uout, st,
@@ -374,6 +390,17 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
   c->have_metric = c->have_prim = false;
   c->launches = 0;
   c->prof = false;
+  {
+    const char* e = std::getenv("HZ_UNFUSED");
+    c->unfused = e && e[0] == '1';
+  }
+  if (cudaFuncSetAttribute(k_substep<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TileGeom<double>::SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(k_substep<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TileGeom<float>::SMEM) != cudaSuccess) {
+    cudaGetLastError();
+    if (c->own) cudaFree(c->base);
+    delete c;
+    return HZ_ECUDA;
+  }
   *out = c;
   return HZ_OK;
 }
@@ -476,7 +503,7 @@ const char* hz_kernel_name(int kind) {
     case K_RHS: return "k_rhs_update";
     case K_C2P: return "k_con2prim";
     case K_GHOST: return "k_fill_ghosts";
-    case K_OTHER: return "other";
+    case K_SUBSTEP: return "k_substep";
     default: return "?";
   }
 }

@@ -1,0 +1,371 @@
+// hz_substep.cuh -- one Runge-Kutta substep as ONE kernel (rows a1-a9 of DESIGN.md section 2).
+//
+// A block owns a tile of TX x TY x TZ cells.  Phase 1: its warps walk the list of the tile's faces
+// (all three directions, each face exactly once) and put the HLLE flux Phi of every
+// face into shared memory; no face value ever goes to HBM.  Phase 2: every cell takes the flux
+// difference of its six faces from shared memory, adds the geometric sources, combines
+// the Runge-Kutta stage, recovers the primitives by Newton-Raphson with the
+// atmosphere floors, and writes U and P -- P also into the ghost cells that mirror this cell
+// (O9), so no separate boundary kernel runs.  P is double-buffered: neighbours still read the
+// old primitives while this block writes the new ones.
+//
+// The face flux is written ONCE, for a sweep along axis 0: a sweep along axis d reads the vector and
+// metric components cyclically rotated by d (and stores the momentum and field fluxes rotated back),
+// which keeps the code a third of the size of three instantiations -- the unfused kernel was bound by
+// instruction-cache misses (profiles/r01_naive.md).
+#pragma once
+#include "hz_kernels.cuh"
+
+namespace hz {
+
+constexpr int SUB_NT = 256;  // threads per block of k_substep
+
+template <typename T> struct Tile;
+// rows of 128 bytes in both precisions
+template <> struct Tile<double> { static constexpr int TX = 16, TY = 8, TZ = 4; };
+template <> struct Tile<float> { static constexpr int TX = 32, TY = 8, TZ = 4; };
+
+template <typename T>
+struct TileGeom {
+  static constexpr int TX = Tile<T>::TX, TY = Tile<T>::TY, TZ = Tile<T>::TZ;
+  static constexpr int NC = TX * TY * TZ;
+  static constexpr int NFX = (TX + 1) * TY * TZ, NFY = TX * (TY + 1) * TZ, NFZ = TX * TY * (TZ + 1);
+  static constexpr int NF = NFX + NFY + NFZ;
+  static constexpr int WX = NFX / 32, WY = NFY / 32, WZ = NFZ / 32;  // warp tasks per direction
+  static_assert(NFX % 32 == 0 && NFY % 32 == 0 && NFZ % 32 == 0, "face lists must split into whole warps");
+  static_assert(NC % SUB_NT == 0, "cells per tile must be a multiple of the block size");
+  static constexpr size_t SMEM = (size_t)NF * NV * sizeof(T);
+};
+
+// packed index of gamma_{(d+a)%3, (d+b)%3} for (a,b) = 00 01 02 11 12 22
+__device__ __forceinline__ int rot6(int d, int a) {
+  // d = 0: 0 1 2 3 4 5;  d = 1: 3 4 1 5 2 0;  d = 2: 5 2 4 0 1 3   (4 bits each)
+  const unsigned tab = d == 0 ? 0x543210u : (d == 1 ? 0x025143u : 0x310425u);
+  return (int)((tab >> (4 * a)) & 15u);
+}
+__device__ __forceinline__ int rot3(int d, int a) { const int s = d + a; return s >= 3 ? s - 3 : s; }
+
+// ---- O1-O3 for one state in the frame of the sweep (axis 0 = sweep axis) ---------------------------
+// q = (rho, ut^0..2, p, B^0..2, psi), m = (alpha, beta^0..2, g00 g01 g02 g11 g12 g22), gi0[k] = gamma^{k0}.
+// U: undensitised conserved; F: coordinate flux along axis 0; lm, lp: coordinate signal speeds.
+template <typename T>
+__device__ __forceinline__ void state_flux0(const T* q, const T* m, const T* gi0, const Par<T>& par,
+                                            T* U, T* F, T& lm, T& lp) {
+  const T* g = m + GXX;
+  T utl[3], Bl[3];
+  lower(g, q + UX, utl);
+  lower(g, q + BX, Bl);
+  const T ut2 = dot3(q + UX, utl);
+  const T W2 = 1 + ut2;
+  const T iW = rsqrt_(W2);
+  const T W = W2 * iW;
+  const T iW2 = iW * iW;
+  const T v2 = ut2 * iW2;
+  const T rhoh = q[RHO] + par.gg1 * q[PR];
+  const T B2 = dot3(q + BX, Bl);
+  const T Bv = dot3(q + BX, utl) * iW;
+  const T b2 = B2 * iW2 + Bv * Bv;
+  const T pstar = q[PR] + b2 * T(0.5);
+  const T Z = rhoh * W2;
+  const T D = q[RHO] * W;
+  const T ZB = Z + B2;
+  const T al = m[AL], be = m[BEX];
+  const T v0 = q[UX] * iW;
+  const T vt = al * v0 - be;
+  const T B0 = q[BX];
+  const T aBd = al * B0 * iW;   // alpha B^0 / W
+  const T WBv = W * Bv;
+  const T ap = al * pstar;
+  U[0] = D;
+  F[0] = D * vt;
+#pragma unroll
+  for (int j = 0; j < 3; j++) {
+    const T vlj = utl[j] * iW;
+    const T Sj = ZB * vlj - Bv * Bl[j];
+    const T bj = Bl[j] * iW + WBv * vlj;
+    U[1 + j] = Sj;
+    F[1 + j] = Sj * vt - bj * aBd;
+  }
+  F[1] += ap;
+  const T tau = Z - q[PR] + (B2 * (1 + v2) - Bv * Bv) * T(0.5) - D;
+  U[4] = tau;
+  F[4] = tau * vt + ap * v0 - al * Bv * B0;
+  const T psi = q[PSI];
+#pragma unroll
+  for (int k = 0; k < 3; k++) U[5 + k] = q[BX + k];
+  U[8] = psi;
+  if (par.cleaning) {
+    const T apsi = al * psi;
+    F[5] = -be * B0 + apsi * gi0[0];
+#pragma unroll
+    for (int k = 1; k < 3; k++) F[5 + k] = vt * q[BX + k] - al * (q[UX + k] * iW) * B0 + apsi * gi0[k];
+    F[8] = al * B0 - be * psi;
+  } else {
+    F[5] = 0;
+#pragma unroll
+    for (int k = 1; k < 3; k++) F[5 + k] = vt * q[BX + k] - (al * (q[UX + k] * iW) - m[BEX + k]) * B0;
+    F[8] = 0;
+  }
+  // fast-speed bound a^2 = c_s^2 + v_A^2 - c_s^2 v_A^2 = (Gamma p + b^2)/(rho h + b^2)   (R7)
+  T a2 = (par.Gam * q[PR] + b2) / (rhoh + b2);
+  a2 = min_(max_(a2, T(0)), T(1));
+  const T den = 1 - v2 * a2;
+  const T disc = a2 * (1 - v2) * (den * gi0[0] - (1 - a2) * v0 * v0);
+  const T sq = sqrt_(max_(disc, T(0)));
+  const T aod = al / den;
+  const T vd = v0 * (1 - a2);
+  lp = aod * (vd + sq) - be;
+  lm = aod * (vd - sq) - be;
+}
+
+// ---- a1-a4 for one face of a sweep along axis d; `id` = cell on the minus side ---------------------
+// Phi comes out in the sweep frame: Phi[1+a] belongs to S_{(d+a)%3}, Phi[5+a] to B^{(d+a)%3}.
+template <typename T>
+__device__ __forceinline__ void face_flux_rot(const Layout& L, const T* __restrict__ P, const T* __restrict__ met,
+                                              long long id, int d, const Par<T>& par, T* Phi) {
+  const long long s = L.stride(d), fs = L.fs;
+  // face metric: mean of the two cells (R8), components rotated into the sweep frame
+  T mf[NM];
+  {
+    const T* a = met + id;
+    mf[AL] = T(0.5) * (a[0] + a[s]);
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+      const T* b = a + (BEX + rot3(d, c)) * fs;
+      mf[BEX + c] = T(0.5) * (b[0] + b[s]);
+    }
+#pragma unroll
+    for (int c = 0; c < 6; c++) {
+      const T* b = a + (GXX + rot6(d, c)) * fs;
+      mf[GXX + c] = T(0.5) * (b[0] + b[s]);
+    }
+  }
+  const T* g = mf + GXX;
+  // first column of the cofactor matrix, determinant, gamma^{k0}
+  const T c0 = g[3] * g[5] - g[4] * g[4];
+  const T c1 = g[4] * g[2] - g[1] * g[5];
+  const T c2 = g[1] * g[4] - g[3] * g[2];
+  const T det = g[0] * c0 + g[1] * c1 + g[2] * c2;
+  const T idet = rcp_(det);
+  const T sqg = sqrt_(det);
+  const T gi0[3] = {c0 * idet, c1 * idet, c2 * idet};
+  // MC reconstruction (O4) of the 9 primitives, rotated
+  T qL[NV], qR[NV];
+#pragma unroll
+  for (int q = 0; q < NV; q++) {
+    const int f = (q >= UX && q <= UZ) ? UX + rot3(d, q - UX) : ((q >= BX && q <= BZ) ? BX + rot3(d, q - BX) : q);
+    const T* a = P + f * fs + id;
+    const T qm = a[-s], q0 = a[0], q1 = a[s], q2 = a[2 * s];
+    qL[q] = q0 + T(0.5) * mc_slope(qm, q0, q1);
+    qR[q] = q1 - T(0.5) * mc_slope(q0, q1, q2);
+  }
+  qL[RHO] = max_(qL[RHO], par.rho_atm); qL[PR] = max_(qL[PR], par.p_atm);
+  qR[RHO] = max_(qR[RHO], par.rho_atm); qR[PR] = max_(qR[PR], par.p_atm);
+  T UL[NV], FL[NV], UR[NV], FR[NV], lmL, lpL, lmR, lpR;
+  state_flux0(qL, mf, gi0, par, UL, FL, lmL, lpL);
+  state_flux0(qR, mf, gi0, par, UR, FR, lmR, lpR);
+  T lp = max_(lpL, lpR), lm = min_(lmL, lmR);
+  if (par.cleaning) {  // light cone of the (B^d, psi) subsystem (O3)
+    const T c = mf[AL] * sqrt_(gi0[0]);
+    lp = max_(lp, c - mf[BEX]);
+    lm = min_(lm, -c - mf[BEX]);
+  }
+  lp = max_(lp, T(0));
+  lm = min_(lm, T(0));
+  const T w = lp - lm;
+  if (w > T(1e-30)) {
+    const T sw = sqg / w, ll = lp * lm;
+#pragma unroll
+    for (int q = 0; q < NV; q++) Phi[q] = sw * (lp * FL[q] - lm * FR[q] + ll * (UR[q] - UL[q]));
+  } else {
+#pragma unroll
+    for (int q = 0; q < NV; q++) Phi[q] = sqg * T(0.5) * (FL[q] + FR[q]);
+  }
+  if (!par.cleaning) Phi[8] = 0;
+}
+
+// ---- a9 fused: store the primitives of cell (i,j,k) and of every ghost cell that mirrors it --------
+template <typename T>
+__device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __restrict__ Pout, int i, int j, int k,
+                                                        const T* q) {
+  const int c3[3] = {i, j, k};
+  int dst[3][3], cnt[3];
+  bool plain = true;
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    const int c = c3[d], n = L.n[d];
+    dst[d][0] = c;
+    cnt[d] = 1;
+    if (L.g[d]) {
+      if (L.bc[d] == 0) {  // periodic wrap
+        if (c < NG) dst[d][cnt[d]++] = c + n;
+        if (c >= n - NG) dst[d][cnt[d]++] = c - n;
+      } else {             // zero gradient: the edge cell fills its ghost layers
+        if (c == 0) { dst[d][1] = -1; dst[d][2] = -2; cnt[d] = 3; }
+        else if (c == n - 1) { dst[d][1] = n; dst[d][2] = n + 1; cnt[d] = 3; }
+      }
+    }
+    plain = plain && cnt[d] == 1;
+  }
+  if (plain) {
+    const long long id = L.idx(i, j, k);
+#pragma unroll
+    for (int v = 0; v < NV; v++) Pout[v * L.fs + id] = q[v];
+    return;
+  }
+  for (int c = 0; c < cnt[2]; c++)
+    for (int b = 0; b < cnt[1]; b++)
+      for (int a = 0; a < cnt[0]; a++) {
+        const long long id = L.idx(dst[0][a], dst[1][b], dst[2][c]);
+#pragma unroll
+        for (int v = 0; v < NV; v++) Pout[v * L.fs + id] = q[v];
+      }
+}
+
+// stage 0: Uout = Uin + dt L;  1: Uout = 3/4 U0 + 1/4 (Uin + dt L);  2: Uout = 1/3 U0 + 2/3 (Uin + dt L)
+template <typename T>
+__global__ void __launch_bounds__(SUB_NT, 1)
+k_substep(Layout L, Par<T> par, const T* __restrict__ P, const T* __restrict__ met, const T* __restrict__ Uin,
+          const T* __restrict__ U0, T* __restrict__ Uout, T* __restrict__ Pout, int stage, T dt,
+          unsigned long long* __restrict__ counters) {
+  using G = TileGeom<T>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* sF = reinterpret_cast<T*>(smem_raw);  // sF[q * NF + face]
+  const int x0 = blockIdx.x * G::TX, y0 = blockIdx.y * G::TY, z0 = blockIdx.z * G::TZ;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+  // ---- phase 1: every face of the tile once ----
+#pragma unroll 1
+  for (int task = warp; task < G::WX + G::WY + G::WZ; task += SUB_NT / 32) {
+    int d = (task >= G::WX) + (task >= G::WX + G::WY);
+    // keep ONE copy of the face-flux body: hide the value of d so the compiler does not clone it per axis
+    asm volatile("" : "+r"(d));
+    const int off = d == 0 ? 0 : (d == 1 ? G::NFX : G::NFX + G::NFY);
+    const int f = task * 32 - off + lane;
+    if (L.g[d] == 0) continue;
+    int a, b, c;  // face coordinates inside the tile; divisions by compile-time constants only
+    if (d == 0) { a = f % (G::TX + 1); const int r = f / (G::TX + 1); b = r % G::TY; c = r / G::TY; }
+    else if (d == 1) { a = f % G::TX; const int r = f / G::TX; b = r % (G::TY + 1); c = r / (G::TY + 1); }
+    else { a = f % G::TX; const int r = f / G::TX; b = r % G::TY; c = r / G::TY; }
+    const int gi = x0 + a, gj = y0 + b, gk = z0 + c;
+    // the face lies between cell (gi,gj,gk) - e_d and cell (gi,gj,gk)
+    const bool valid = gi < L.n[0] + (d == 0) && gj < L.n[1] + (d == 1) && gk < L.n[2] + (d == 2);
+    if (!valid) continue;
+    const long long id = L.idx(gi, gj, gk) - L.stride(d);
+    T Phi[NV];
+    face_flux_rot<T>(L, P, met, id, d, par, Phi);
+    T* o = sF + off + f;
+    o[0] = Phi[0];
+    o[4 * G::NF] = Phi[4];
+    o[8 * G::NF] = Phi[8];
+#pragma unroll
+    for (int c3 = 0; c3 < 3; c3++) {
+      const int t = rot3(d, c3);
+      o[(1 + t) * G::NF] = Phi[1 + c3];
+      o[(5 + t) * G::NF] = Phi[5 + c3];
+    }
+  }
+  __syncthreads();
+
+  // ---- phase 2: per cell ----
+  int fail = 0, reset = 0, pfl = 0, it = 0;
+#pragma unroll 1
+  for (int cidx = threadIdx.x; cidx < G::NC; cidx += SUB_NT) {
+    const int a = cidx % G::TX, r = cidx / G::TX;
+    const int b = r % G::TY, c = r / G::TY;
+    const int i = x0 + a, j = y0 + b, k = z0 + c;
+    if (i >= L.n[0] || j >= L.n[1] || k >= L.n[2]) continue;
+    const long long id = L.idx(i, j, k);
+    T R[NV];
+#pragma unroll
+    for (int q = 0; q < NV; q++) R[q] = 0;
+    if (L.g[0]) {
+      const T ih = T(1.0 / L.h[0]);
+      const T* o = sF + (c * G::TY + b) * (G::TX + 1) + a;
+#pragma unroll
+      for (int q = 0; q < NV; q++) R[q] -= (o[q * G::NF + 1] - o[q * G::NF]) * ih;
+    }
+    if (L.g[1]) {
+      const T ih = T(1.0 / L.h[1]);
+      const T* o = sF + G::NFX + (c * (G::TY + 1) + b) * G::TX + a;
+#pragma unroll
+      for (int q = 0; q < NV; q++) R[q] -= (o[q * G::NF + G::TX] - o[q * G::NF]) * ih;
+    }
+    if (L.g[2]) {
+      const T ih = T(1.0 / L.h[2]);
+      const T* o = sF + G::NFX + G::NFY + (c * G::TY + b) * G::TX + a;
+#pragma unroll
+      for (int q = 0; q < NV; q++) R[q] -= (o[q * G::NF + G::TX * G::TY] - o[q * G::NF]) * ih;
+    }
+    T q[NV];
+    load_fields(P, L.fs, id, NV, q);
+    add_sources(L, met, id, q, par, R);
+    // a7: Runge-Kutta stage combine
+    T u[NV];
+#pragma unroll
+    for (int v = 0; v < NV; v++) {
+      T u1 = Uin[v * L.fs + id] + dt * R[v];
+      if (stage == 1) u1 = T(0.75) * U0[v * L.fs + id] + T(0.25) * u1;
+      if (stage == 2) u1 = T(1.0 / 3.0) * U0[v * L.fs + id] + T(2.0 / 3.0) * u1;
+      u[v] = u1;
+    }
+    // a8: primitive recovery and floors
+    T m[NM];
+    load_fields(met, L.fs, id, NM, m);
+    T cf[6], gi[6];
+    const T det = cofactors(m + GXX, cf);
+    const T sq = sqrt_(det);
+    const T idet = rcp_(det);
+#pragma unroll
+    for (int a6 = 0; a6 < 6; a6++) gi[a6] = cf[a6] * idet;
+    T w[NV];
+#pragma unroll
+    for (int v = 0; v < NV; v++) w[v] = u[v] / sq;
+    if (!par.cleaning) w[8] = 0;
+    T Zg;
+    {  // guess from the previous primitives of this cell
+      T utl[3];
+      lower(m + GXX, q + UX, utl);
+      const T W2 = 1 + dot3(q + UX, utl);
+      Zg = (q[RHO] + par.gg1 * q[PR]) * W2;
+    }
+    T qn[NV];
+    int its = 0;
+    const int fl = con2prim(w, m, gi, par, Zg, qn, its);
+    it = its > it ? its : it;
+    bool rs = fl != 0;
+    if (!rs && qn[RHO] < par.rho_thr) rs = true;
+    bool pf = false;
+    if (rs) {
+      qn[RHO] = par.rho_atm; qn[PR] = par.p_atm;
+#pragma unroll
+      for (int a3 = 0; a3 < 3; a3++) { qn[UX + a3] = 0; qn[BX + a3] = w[5 + a3]; }
+      qn[PSI] = w[8];
+    } else if (qn[PR] < par.p_atm) {
+      pf = true;
+      qn[PR] = par.p_atm;
+    }
+    if (rs || pf) {
+      T un[NV];
+      prim2con(qn, m, par, un);
+#pragma unroll
+      for (int v = 0; v < NV; v++) u[v] = sq * un[v];
+    }
+    fail += fl != 0; reset += rs; pfl += pf;
+#pragma unroll
+    for (int v = 0; v < NV; v++) Uout[v * L.fs + id] = u[v];
+    store_prims_with_images(L, Pout, i, j, k, qn);
+  }
+  // warp-level reduction of the counters: [0] c2p_fail, [1] atm_reset, [2] p_floor, [3] max iterations
+  const unsigned full = 0xffffffffu;
+  const int nf = __reduce_add_sync(full, fail), nr = __reduce_add_sync(full, reset), np = __reduce_add_sync(full, pfl);
+  const int mi = __reduce_max_sync(full, it);
+  if (lane == 0) {
+    if (nf) atomicAdd(counters + 0, (unsigned long long)nf);
+    if (nr) atomicAdd(counters + 1, (unsigned long long)nr);
+    if (np) atomicAdd(counters + 2, (unsigned long long)np);
+    if ((unsigned long long)mi > counters[3]) atomicMax(counters + 3, (unsigned long long)mi);
+  }
+}
+
+}  // namespace hz
