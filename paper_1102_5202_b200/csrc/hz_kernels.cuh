@@ -1,15 +1,14 @@
 // hz_kernels.cuh -- the kernels of one Runge-Kutta substep and of the set/get/diagnostic calls.
 //
-// Substep = k_rhs_update (reconstruction, HLLE fluxes, flux difference, sources, RK combine:
-// PAPER.md:76-80) -> k_con2prim (Newton-Raphson recovery + floors) -> k_fill_ghosts.
-// All kernels are templated on the arithmetic type (double / float).
+// The substep itself is the one fused kernel of hz_substep.cuh; here are the ghost fill used by
+// hz_set_metric / hz_set_primitives, the pack / unpack kernels of the set / get calls and the
+// reductions of hz_diagnostics.  All kernels are templated on the arithmetic type (double / float).
 #pragma once
 #include "hz_layout.cuh"
 #include "hz_physics.cuh"
 
 namespace hz {
 
-constexpr int BLK = 128;       // threads per block of the per-cell kernels
 constexpr int NDIAG = 16;      // doubles per block partial of the diagnostics reduction
 
 // interior linear index -> (i, j, k), x fastest
@@ -149,189 +148,6 @@ __global__ void k_unpack_fields(Layout L, const T* __restrict__ F, int f0, int n
   cell_of(L, t, i, j, k);
   const long long id = L.idx(i, j, k);
   for (int f = 0; f < nf; f++) out[f * n + t] = F[(f0 + f) * L.fs + id];
-}
-
-// ---- a1-a5 for one face: MC reconstruction of the 9 primitives, face metric, HLLE ---------------
-// `id` is the cell on the minus side of the face.
-template <typename T, int D>
-__device__ __forceinline__ void face_flux(const Layout& L, const T* __restrict__ P, const T* __restrict__ met,
-                                          long long id, const Par<T>& par, T* Phi) {
-  const long long s = L.stride(D);
-  T qL[NV], qR[NV];
-#pragma unroll
-  for (int q = 0; q < NV; q++) {
-    const T* a = P + q * L.fs + id;
-    const T qm = a[-s], q0 = a[0], q1 = a[s], q2 = a[2 * s];
-    qL[q] = q0 + T(0.5) * mc_slope(qm, q0, q1);
-    qR[q] = q1 - T(0.5) * mc_slope(q0, q1, q2);
-  }
-  T mf[NM];
-#pragma unroll
-  for (int c = 0; c < NM; c++) mf[c] = T(0.5) * (met[c * L.fs + id] + met[c * L.fs + id + s]);
-  hlle_face<T, D>(qL, qR, mf, par, Phi);
-}
-
-template <typename T, int D>
-__device__ __forceinline__ void flux_difference(const Layout& L, const T* __restrict__ P, const T* __restrict__ met,
-                                                long long id, const Par<T>& par, T* R) {
-  T Pp[NV], Pm[NV];
-  face_flux<T, D>(L, P, met, id, par, Pp);
-  face_flux<T, D>(L, P, met, id - L.stride(D), par, Pm);
-  const T ih = T(1.0 / L.h[D]);
-#pragma unroll
-  for (int q = 0; q < NV; q++) R[q] -= (Pp[q] - Pm[q]) * ih;
-}
-
-// ---- a6: metric derivatives, fluid and cleaning sources at a cell ---------------------------------
-template <typename T>
-__device__ __forceinline__ void add_sources(const Layout& L, const T* __restrict__ met, long long id, const T* q,
-                                            const Par<T>& par, T* R) {
-  T m[NM];
-  load_fields(met, L.fs, id, NM, m);
-  T c[6], gi[6];
-  const T det = cofactors(m + GXX, c);
-  const T sq = sqrt_(det);
-  const T idet = rcp_(det);
-#pragma unroll
-  for (int a = 0; a < 6; a++) gi[a] = c[a] * idet;
-  T dm[3][NM];
-  T dQ[3] = {0, 0, 0};  // sum_j d_j(alpha sqrt(gamma) gamma^{kj})
-  T dRb = 0;            // sum_j d_j(sqrt(gamma) beta^j)
-#pragma unroll
-  for (int d = 0; d < 3; d++) {
-    if (L.g[d] == 0) {
-#pragma unroll
-      for (int a = 0; a < NM; a++) dm[d][a] = 0;
-      continue;
-    }
-    const long long s = L.stride(d);
-    const T i2h = T(1.0 / (2 * L.h[d]));
-    T mp[NM], mm[NM];
-    load_fields(met, L.fs, id + s, NM, mp);
-    load_fields(met, L.fs, id - s, NM, mm);
-#pragma unroll
-    for (int a = 0; a < NM; a++) dm[d][a] = (mp[a] - mm[a]) * i2h;
-    if (par.cleaning) {
-      T cp[6], cm[6];
-      const T dp = cofactors(mp + GXX, cp), dn = cofactors(mm + GXX, cm);
-      const T sp = sqrt_(dp), sm = sqrt_(dn);
-      const T ap = mp[AL] / sp, am = mm[AL] / sm;  // alpha sqrt(gamma) gamma^{kd} = alpha cof_kd / sqrt(gamma)
-#pragma unroll
-      for (int k = 0; k < 3; k++) dQ[k] += (ap * cp[sym(k, d)] - am * cm[sym(k, d)]) * i2h;
-      dRb += (sp * mp[BEX + d] - sm * mm[BEX + d]) * i2h;
-    }
-  }
-  fluid_source(q, m, dm, par, gi, sq, R);
-  if (par.cleaning) {  // cleaning sources (R14), not multiplied by alpha
-#pragma unroll
-    for (int k = 0; k < 3; k++) {
-      T adv = q[BX] * dm[0][BEX + k] + q[BY] * dm[1][BEX + k] + q[BZ] * dm[2][BEX + k];
-      R[5 + k] += -sq * adv + q[PSI] * dQ[k];
-    }
-    T Bda = q[BX] * dm[0][AL] + q[BY] * dm[1][AL] + q[BZ] * dm[2][AL];
-    R[8] += sq * Bda - q[PSI] * dRb - m[AL] * par.kappa * sq * q[PSI];
-  } else {
-    R[8] = 0;
-  }
-}
-
-// ---- a1-a7: L(U) of one cell and the Runge-Kutta stage combine (O7) ---------------------
-// stage 0: Uout = Uin + dt L;  1: Uout = 3/4 U0 + 1/4 (Uin + dt L);  2: Uout = 1/3 U0 + 2/3 (Uin + dt L)
-template <typename T>
-__global__ void __launch_bounds__(BLK) k_rhs_update(Layout L, Par<T> par, const T* __restrict__ P,
-                                                    const T* __restrict__ met, const T* __restrict__ Uin,
-                                                    const T* __restrict__ U0, T* __restrict__ Uout, int stage, T dt) {
-  const long long n = L.ncell();
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= n) return;
-  int i, j, k;
-  cell_of(L, t, i, j, k);
-  const long long id = L.idx(i, j, k);
-  T R[NV];
-#pragma unroll
-  for (int q = 0; q < NV; q++) R[q] = 0;
-  if (L.g[0]) flux_difference<T, 0>(L, P, met, id, par, R);
-  if (L.g[1]) flux_difference<T, 1>(L, P, met, id, par, R);
-  if (L.g[2]) flux_difference<T, 2>(L, P, met, id, par, R);
-  T q[NV];
-  load_fields(P, L.fs, id, NV, q);
-  add_sources(L, met, id, q, par, R);
-#pragma unroll
-  for (int v = 0; v < NV; v++) {
-    T u1 = Uin[v * L.fs + id] + dt * R[v];
-    if (stage == 1) u1 = T(0.75) * U0[v * L.fs + id] + T(0.25) * u1;
-    if (stage == 2) u1 = T(1.0 / 3.0) * U0[v * L.fs + id] + T(2.0 / 3.0) * u1;
-    Uout[v * L.fs + id] = u1;
-  }
-}
-
-// ---- a8: Newton-Raphson recovery + floors; U is rewritten where a floor acted ---------------------
-// counters: [0] c2p_fail, [1] atm_reset, [2] p_floor, [3] max iterations seen
-template <typename T>
-__global__ void __launch_bounds__(BLK) k_con2prim(Layout L, Par<T> par, T* __restrict__ U, const T* __restrict__ met,
-                                                  T* __restrict__ P, unsigned long long* __restrict__ counters) {
-  const long long n = L.ncell();
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const bool active = t < n;
-  int fail = 0, reset = 0, pfl = 0, it = 0;
-  if (active) {
-    int i, j, k;
-    cell_of(L, t, i, j, k);
-    const long long id = L.idx(i, j, k);
-    T m[NM];
-    load_fields(met, L.fs, id, NM, m);
-    T c[6], gi[6];
-    const T det = cofactors(m + GXX, c);
-    const T sq = sqrt_(det);
-    const T idet = rcp_(det);
-#pragma unroll
-    for (int a = 0; a < 6; a++) gi[a] = c[a] * idet;
-    T w[NV];
-#pragma unroll
-    for (int v = 0; v < NV; v++) w[v] = U[v * L.fs + id] / sq;
-    if (!par.cleaning) w[8] = 0;
-    T old[NV];
-    load_fields(P, L.fs, id, NV, old);
-    T Zg;
-    {  // guess from the previous primitives of this cell
-      T utl[3];
-      lower(m + GXX, old + UX, utl);
-      T W2 = 1 + dot3(old + UX, utl);
-      Zg = old[RHO] * (1 + par.gg1 * old[PR] / old[RHO]) * W2;
-    }
-    T q[NV];
-    fail = con2prim(w, m, gi, par, Zg, q, it);
-    if (fail) reset = 1;
-    else if (q[RHO] < par.rho_thr) reset = 1;
-    if (reset) {
-      q[RHO] = par.rho_atm; q[PR] = par.p_atm;
-#pragma unroll
-      for (int a = 0; a < 3; a++) { q[UX + a] = 0; q[BX + a] = w[5 + a]; }
-      q[PSI] = w[8];
-    } else if (q[PR] < par.p_atm) {
-      pfl = 1;
-      q[PR] = par.p_atm;
-    }
-#pragma unroll
-    for (int v = 0; v < NV; v++) P[v * L.fs + id] = q[v];
-    if (reset || pfl) {
-      T u[NV];
-      prim2con(q, m, par, u);
-#pragma unroll
-      for (int v = 0; v < NV; v++) U[v * L.fs + id] = sq * u[v];
-    }
-  }
-  // warp-level reduction of the counters
-  const unsigned full = 0xffffffffu;
-  const int nf = __popc(__ballot_sync(full, fail)), nr = __popc(__ballot_sync(full, reset)),
-            np = __popc(__ballot_sync(full, pfl));
-  const int mi = __reduce_max_sync(full, it);
-  if ((threadIdx.x & 31) == 0) {
-    if (nf) atomicAdd(counters + 0, (unsigned long long)nf);
-    if (nr) atomicAdd(counters + 1, (unsigned long long)nr);
-    if (np) atomicAdd(counters + 2, (unsigned long long)np);
-    if ((unsigned long long)mi > counters[3]) atomicMax(counters + 3, (unsigned long long)mi);
-  }
 }
 
 // ---- a10: global reductions with warp shuffles ---------------------------------

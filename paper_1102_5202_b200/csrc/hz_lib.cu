@@ -102,7 +102,7 @@ struct hz_ctx {
   int pcur;   // P[pcur] holds the current primitives
   int stage;  // next Runge-Kutta stage 0, 1, 2
   bool have_metric, have_prim;
-  bool unfused;  // HZ_UNFUSED=1 in the environment at hz_create: the first, three-kernel path (A/B timing only)
+  CUtensorMap tmP[2], tmM;  // TMA descriptors of the two primitive sets and of the metric (k_substep stage-in)
   long long launches;
   bool prof;                          // per-kernel event timing on (hz_profile)
   std::vector<cudaEvent_t> ev_pool;   // pairs: [2i] start, [2i+1] stop
@@ -137,7 +137,7 @@ Par<T> make_par(const hz_ctx* c) {
   return p;
 }
 
-enum { K_RHS = 0, K_C2P = 1, K_GHOST = 2, K_SUBSTEP = 3 };
+enum { K_SUBSTEP = 0, K_GHOST = 1, K_RESERVED2 = 2, K_RESERVED3 = 3 };
 constexpr size_t PROF_MAX = 16384;
 
 // Brackets one launch with events when profiling is on.
@@ -239,42 +239,63 @@ int set_prims_t(hz_ctx* c, const void* prim8) {
 template <typename T>
 int substep_t(hz_ctx* c, double dt) {
   const Layout& L = c->L;
-  const long long n = L.ncell();
   const Par<T> par = make_par<T>(c);
   const int st = c->stage;
   const T* Uin = c->U<T>(c->cur);
   T* Uout = st == 0 ? c->U<T>(1 - c->cur) : c->U<T>(c->cur);
   const T* U0 = st == 0 ? Uin : c->U<T>(c->u0);
-  if (!c->unfused) {  // the whole substep in one kernel (hz_substep.cuh)
-    using G = TileGeom<T>;
-    const dim3 grid((L.n[0] + G::TX - 1) / G::TX, (L.n[1] + G::TY - 1) / G::TY, (L.n[2] + G::TZ - 1) / G::TZ);
-    {
-      ProfScope ps(c, K_SUBSTEP);
-      k_substep<T><<<grid, SUB_NT, G::SMEM, c->stream>>>(L, par, c->P<T>(c->pcur), c->met<T>(), Uin, U0, Uout,
-                                                          c->P<T>(1 - c->pcur), st, (T)dt, c->counters());
-    }
-    HZ_LAUNCHED(c);
-    if (st == 0) { c->u0 = c->cur; c->cur = 1 - c->cur; }
-    c->pcur = 1 - c->pcur;
-    c->stage = (st + 1) % 3;
-    return HZ_OK;
-  }
+  using G = TileGeom<T>;
+  const dim3 grid((L.n[0] + G::TX - 1) / G::TX, (L.n[1] + G::TY - 1) / G::TY, (L.n[2] + G::TZ - 1) / G::TZ);
   {
-    ProfScope ps(c, K_RHS);
-    k_rhs_update<T><<<nblocks(n, BLK), BLK, 0, c->stream>>>(L, par, c->P<T>(c->pcur), c->met<T>(), Uin, U0, Uout, st,
-                                                            (T)dt);
+    ProfScope ps(c, K_SUBSTEP);
+    k_substep<T><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, Uin, U0, Uout,
+                                                        c->P<T>(1 - c->pcur), st, (T)dt, c->counters());
   }
   HZ_LAUNCHED(c);
   if (st == 0) { c->u0 = c->cur; c->cur = 1 - c->cur; }
-  {
-    ProfScope ps(c, K_C2P);
-    k_con2prim<T><<<nblocks(n, BLK), BLK, 0, c->stream>>>(L, par, c->U<T>(c->cur), c->met<T>(), c->P<T>(c->pcur),
-                                                          c->counters());
-  }
-  HZ_LAUNCHED(c);
-  int rc;
-  if ((rc = fill_ghosts_P<T>(c))) return rc;
+  c->pcur = 1 - c->pcur;
   c->stage = (st + 1) % 3;
+  return HZ_OK;
+}
+
+// Tensor map of a padded SoA field set as a 4D array (x, y, z, field) with the staging box of k_substep.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+template <typename T>
+int make_tensor_map(const Layout& L, void* base, int nfields, int by, int bz, CUtensorMap* out) {
+  static EncodeTiledFn encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) {
+      cudaGetLastError();
+      return HZ_ECUDA;
+    }
+    encode = (EncodeTiledFn)fn;
+  }
+  using G = TileGeom<T>;
+  const cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.N[1], (cuuint64_t)L.N[2], (cuuint64_t)nfields};
+  const cuuint64_t strides[3] = {(cuuint64_t)L.pitch * sizeof(T), (cuuint64_t)L.sz * sizeof(T),
+                                 (cuuint64_t)L.fs * sizeof(T)};
+  const cuuint32_t box[4] = {(cuuint32_t)G::BX, (cuuint32_t)by, (cuuint32_t)bz, (cuuint32_t)nfields};
+  const cuuint32_t es[4] = {1, 1, 1, 1};
+  const CUresult r = encode(out, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4,
+                            base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? HZ_OK : HZ_ECUDA;
+}
+template <typename T>
+int make_maps_t(hz_ctx* c) {
+  using G = TileGeom<T>;
+  int rc;
+  for (int w = 0; w < 2; w++)
+    if ((rc = make_tensor_map<T>(c->L, c->P<T>(w), NV, G::BY, G::BZ, &c->tmP[w]))) return rc;
+  if ((rc = make_tensor_map<T>(c->L, c->met<T>(), NM, G::MY, G::MZ, &c->tmM))) return rc;
+  if (cudaFuncSetAttribute(k_substep<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM) != cudaSuccess) {
+    cudaGetLastError();
+    return HZ_ECUDA;
+  }
   return HZ_OK;
 }
 
@@ -390,13 +411,7 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
   c->have_metric = c->have_prim = false;
   c->launches = 0;
   c->prof = false;
-  {
-    const char* e = std::getenv("HZ_UNFUSED");
-    c->unfused = e && e[0] == '1';
-  }
-  if (cudaFuncSetAttribute(k_substep<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TileGeom<double>::SMEM) != cudaSuccess ||
-      cudaFuncSetAttribute(k_substep<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TileGeom<float>::SMEM) != cudaSuccess) {
-    cudaGetLastError();
+  if (HZ_DISPATCH(c, make_maps_t, c) != HZ_OK) {
     if (c->own) cudaFree(c->base);
     delete c;
     return HZ_ECUDA;
@@ -500,10 +515,9 @@ int hz_profile_read(hz_ctx* c, double* ms, long long* launches) {
 
 const char* hz_kernel_name(int kind) {
   switch (kind) {
-    case K_RHS: return "k_rhs_update";
-    case K_C2P: return "k_con2prim";
-    case K_GHOST: return "k_fill_ghosts";
     case K_SUBSTEP: return "k_substep";
+    case K_GHOST: return "k_fill_ghosts";
+    case K_RESERVED2: case K_RESERVED3: return "-";
     default: return "?";
   }
 }

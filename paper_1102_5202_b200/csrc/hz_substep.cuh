@@ -1,40 +1,59 @@
 // hz_substep.cuh -- one Runge-Kutta substep as ONE kernel (rows a1-a9 of DESIGN.md section 2).
 //
-// A block owns a tile of TX x TY x TZ cells.  Phase 1: its warps walk the list of the tile's faces
-// (all three directions, each face exactly once) and put the HLLE flux Phi of every
-// face into shared memory; no face value ever goes to HBM.  Phase 2: every cell takes the flux
-// difference of its six faces from shared memory, adds the geometric sources, combines
-// the Runge-Kutta stage, recovers the primitives by Newton-Raphson with the
-// atmosphere floors, and writes U and P -- P also into the ghost cells that mirror this cell
-// (O9), so no separate boundary kernel runs.  P is double-buffered: neighbours still read the
-// old primitives while this block writes the new ones.
+// A block owns a tile of TX x TY x TZ cells.
+//   Stage-in : one thread issues two TMA box loads (cp.async.bulk.tensor.4d): the 9 primitives of the
+//              tile with a 2-cell halo and the 10 metric components with a 1-cell halo (2 in x, so
+//              both boxes share the x origin) land in shared memory; everyone waits on one mbarrier.
+//   Phase 1  : the warps walk the list of the tile's faces (all three directions, each face exactly
+//              once): MC reconstruction, face metric, left/right states, HLLE.  The
+//              flux Phi of every face goes to shared memory; no face value ever goes to HBM.
+//   Phase 2  : every cell takes the flux difference of its six faces from shared memory, adds the
+//              geometric sources, combines the Runge-Kutta stage, recovers the
+//              primitives by Newton-Raphson with the atmosphere floors, and writes U and
+//              P -- P also into the ghost cells that mirror this cell (O9), so no separate
+//              boundary kernel runs.  P is double-buffered: neighbours still read the old primitives
+//              while this block writes the new ones.
 //
 // The face flux is written ONCE, for a sweep along axis 0: a sweep along axis d reads the vector and
 // metric components cyclically rotated by d (and stores the momentum and field fluxes rotated back),
 // which keeps the code a third of the size of three instantiations -- the unfused kernel was bound by
 // instruction-cache misses (profiles/r01_naive.md).
 #pragma once
+#include <cuda.h>  // CUtensorMap (type only; the encoder is fetched through the runtime, see hz_lib.cu)
+
 #include "hz_kernels.cuh"
 
 namespace hz {
 
-constexpr int SUB_NT = 256;  // threads per block of k_substep
-
+// Tile shape, threads per block (= cells per tile) and x halo of the staged boxes.  TMA wants the first
+// element of every box row on a 16-byte boundary, so the x halo is 16 bytes: 2 doubles or 4 floats.
 template <typename T> struct Tile;
-// rows of 128 bytes in both precisions
-template <> struct Tile<double> { static constexpr int TX = 16, TY = 8, TZ = 4; };
-template <> struct Tile<float> { static constexpr int TX = 32, TY = 8, TZ = 4; };
+template <> struct Tile<double> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = 256, HX = 2; };
+template <> struct Tile<float> { static constexpr int TX = 16, TY = 8, TZ = 4, NT = 512, HX = 4; };
 
 template <typename T>
 struct TileGeom {
-  static constexpr int TX = Tile<T>::TX, TY = Tile<T>::TY, TZ = Tile<T>::TZ;
+  static constexpr int TX = Tile<T>::TX, TY = Tile<T>::TY, TZ = Tile<T>::TZ, NT = Tile<T>::NT, HX = Tile<T>::HX;
   static constexpr int NC = TX * TY * TZ;
   static constexpr int NFX = (TX + 1) * TY * TZ, NFY = TX * (TY + 1) * TZ, NFZ = TX * TY * (TZ + 1);
   static constexpr int NF = NFX + NFY + NFZ;
   static constexpr int WX = NFX / 32, WY = NFY / 32, WZ = NFZ / 32;  // warp tasks per direction
   static_assert(NFX % 32 == 0 && NFY % 32 == 0 && NFZ % 32 == 0, "face lists must split into whole warps");
-  static_assert(NC % SUB_NT == 0, "cells per tile must be a multiple of the block size");
-  static constexpr size_t SMEM = (size_t)NF * NV * sizeof(T);
+  static_assert(NC == NT, "phase 2 maps one cell to one thread");
+  static_assert(HX >= NG && (HX * sizeof(T)) % 16 == 0, "x halo: at least NG cells and 16-byte box rows starts");
+  // staged boxes: primitives with halo 2, metric with halo 1; both with halo HX along x (same x origin)
+  static constexpr int BX = TX + 2 * HX, BY = TY + 2 * NG, BZ = TZ + 2 * NG;
+  static constexpr int MY = TY + 2, MZ = TZ + 2;
+  static constexpr int PFS = BX * BY * BZ;  // field stride of the staged primitives
+  static constexpr int MFS = BX * MY * MZ;  // field stride of the staged metric
+  static_assert((BX * sizeof(T)) % 16 == 0, "TMA box rows must be multiples of 16 bytes");
+  static constexpr size_t align128(size_t x) { return (x + 127) / 128 * 128; }
+  static constexpr size_t OFF_P = 0;
+  static constexpr size_t OFF_M = align128(OFF_P + (size_t)NV * PFS * sizeof(T));
+  static constexpr size_t OFF_F = align128(OFF_M + (size_t)NM * MFS * sizeof(T));
+  static constexpr size_t OFF_BAR = align128(OFF_F + (size_t)NV * NF * sizeof(T));
+  static constexpr size_t SMEM = OFF_BAR + 16;
+  static constexpr unsigned TX_BYTES = (unsigned)((NV * PFS + NM * MFS) * sizeof(T));
 };
 
 // packed index of gamma_{(d+a)%3, (d+b)%3} for (a,b) = 00 01 02 11 12 22
@@ -44,6 +63,34 @@ __device__ __forceinline__ int rot6(int d, int a) {
   return (int)((tab >> (4 * a)) & 15u);
 }
 __device__ __forceinline__ int rot3(int d, int a) { const int s = d + a; return s >= 3 ? s - 3 : s; }
+
+// ---- TMA + mbarrier (sm_90+ PTX; SASS: UTMALDG, SYNCS) ---------------------------------------------
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  unsigned done = 0;
+  while (!done) {
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  }
+}
+// 4D box (x, y, z, field) of a padded SoA array -> shared memory, completion on `bar`
+__device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1, int c2,
+                                            int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+      ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+      : "memory");
+}
 
 // ---- O1-O3 for one state in the frame of the sweep (axis 0 = sweep axis) ---------------------------
 // q = (rho, ut^0..2, p, B^0..2, psi), m = (alpha, beta^0..2, g00 g01 g02 g11 g12 g22), gi0[k] = gamma^{k0}.
@@ -118,27 +165,26 @@ __device__ __forceinline__ void state_flux0(const T* q, const T* m, const T* gi0
   lm = aod * (vd - sq) - be;
 }
 
-// ---- a1-a4 for one face of a sweep along axis d; `id` = cell on the minus side ---------------------
+// ---- a1-a4 for one face of a sweep along axis d, everything read from the staged tile ---------------
+// sPc / sMc: staged primitives / metric at the cell on the MINUS side of the face (field 0);
+// sp / sm: element stride of axis d inside the two boxes.
 // Phi comes out in the sweep frame: Phi[1+a] belongs to S_{(d+a)%3}, Phi[5+a] to B^{(d+a)%3}.
 template <typename T>
-__device__ __forceinline__ void face_flux_rot(const Layout& L, const T* __restrict__ P, const T* __restrict__ met,
-                                              long long id, int d, const Par<T>& par, T* Phi) {
-  const long long s = L.stride(d), fs = L.fs;
+__device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T* __restrict__ sMc, int sp, int sm,
+                                              int d, const Par<T>& par, T* Phi) {
+  using G = TileGeom<T>;
   // face metric: mean of the two cells (R8), components rotated into the sweep frame
   T mf[NM];
-  {
-    const T* a = met + id;
-    mf[AL] = T(0.5) * (a[0] + a[s]);
+  mf[AL] = T(0.5) * (sMc[0] + sMc[sm]);
 #pragma unroll
-    for (int c = 0; c < 3; c++) {
-      const T* b = a + (BEX + rot3(d, c)) * fs;
-      mf[BEX + c] = T(0.5) * (b[0] + b[s]);
-    }
+  for (int c = 0; c < 3; c++) {
+    const T* b = sMc + (BEX + rot3(d, c)) * G::MFS;
+    mf[BEX + c] = T(0.5) * (b[0] + b[sm]);
+  }
 #pragma unroll
-    for (int c = 0; c < 6; c++) {
-      const T* b = a + (GXX + rot6(d, c)) * fs;
-      mf[GXX + c] = T(0.5) * (b[0] + b[s]);
-    }
+  for (int c = 0; c < 6; c++) {
+    const T* b = sMc + (GXX + rot6(d, c)) * G::MFS;
+    mf[GXX + c] = T(0.5) * (b[0] + b[sm]);
   }
   const T* g = mf + GXX;
   // first column of the cofactor matrix, determinant, gamma^{k0}
@@ -154,8 +200,8 @@ __device__ __forceinline__ void face_flux_rot(const Layout& L, const T* __restri
 #pragma unroll
   for (int q = 0; q < NV; q++) {
     const int f = (q >= UX && q <= UZ) ? UX + rot3(d, q - UX) : ((q >= BX && q <= BZ) ? BX + rot3(d, q - BX) : q);
-    const T* a = P + f * fs + id;
-    const T qm = a[-s], q0 = a[0], q1 = a[s], q2 = a[2 * s];
+    const T* a = sPc + f * G::PFS;
+    const T qm = a[-sp], q0 = a[0], q1 = a[sp], q2 = a[2 * sp];
     qL[q] = q0 + T(0.5) * mc_slope(qm, q0, q1);
     qR[q] = q1 - T(0.5) * mc_slope(q0, q1, q2);
   }
@@ -182,6 +228,53 @@ __device__ __forceinline__ void face_flux_rot(const Layout& L, const T* __restri
     for (int q = 0; q < NV; q++) Phi[q] = sqg * T(0.5) * (FL[q] + FR[q]);
   }
   if (!par.cleaning) Phi[8] = 0;
+}
+
+// ---- a6 from the staged metric: centred differences, fluid and cleaning sources at a cell ----------
+// sMc: staged metric at the cell (field 0).  Same arithmetic as add_sources (hz_kernels.cuh).
+template <typename T>
+__device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __restrict__ sMc, const T* m, const T* q,
+                                                   const Par<T>& par, const T* gi, T sq, T* R) {
+  using G = TileGeom<T>;
+  T dm[3][NM];
+  T dQ[3] = {0, 0, 0};  // sum_j d_j(alpha sqrt(gamma) gamma^{kj})
+  T dRb = 0;            // sum_j d_j(sqrt(gamma) beta^j)
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    if (L.g[d] == 0) {
+#pragma unroll
+      for (int a = 0; a < NM; a++) dm[d][a] = 0;
+      continue;
+    }
+    const int s = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::MY);
+    const T i2h = T(1.0 / (2 * L.h[d]));
+    T mp[NM], mm[NM];
+#pragma unroll
+    for (int a = 0; a < NM; a++) { mp[a] = sMc[a * G::MFS + s]; mm[a] = sMc[a * G::MFS - s]; }
+#pragma unroll
+    for (int a = 0; a < NM; a++) dm[d][a] = (mp[a] - mm[a]) * i2h;
+    if (par.cleaning) {
+      T cp[6], cm[6];
+      const T dp = cofactors(mp + GXX, cp), dn = cofactors(mm + GXX, cm);
+      const T sp = sqrt_(dp), sn = sqrt_(dn);
+      const T ap = mp[AL] / sp, am = mm[AL] / sn;  // alpha sqrt(gamma) gamma^{kd} = alpha cof_kd / sqrt(gamma)
+#pragma unroll
+      for (int k = 0; k < 3; k++) dQ[k] += (ap * cp[sym(k, d)] - am * cm[sym(k, d)]) * i2h;
+      dRb += (sp * mp[BEX + d] - sn * mm[BEX + d]) * i2h;
+    }
+  }
+  fluid_source(q, m, dm, par, gi, sq, R);
+  if (par.cleaning) {  // cleaning sources (R14), not multiplied by alpha
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+      const T adv = q[BX] * dm[0][BEX + k] + q[BY] * dm[1][BEX + k] + q[BZ] * dm[2][BEX + k];
+      R[5 + k] += -sq * adv + q[PSI] * dQ[k];
+    }
+    const T Bda = q[BX] * dm[0][AL] + q[BY] * dm[1][AL] + q[BZ] * dm[2][AL];
+    R[8] += sq * Bda - q[PSI] * dRb - m[AL] * par.kappa * sq * q[PSI];
+  } else {
+    R[8] = 0;
+  }
 }
 
 // ---- a9 fused: store the primitives of cell (i,j,k) and of every ghost cell that mirrors it --------
@@ -223,20 +316,41 @@ __device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __re
 }
 
 // stage 0: Uout = Uin + dt L;  1: Uout = 3/4 U0 + 1/4 (Uin + dt L);  2: Uout = 1/3 U0 + 2/3 (Uin + dt L)
+// tmP / tmM: tensor maps of the current primitives and of the metric as 4D arrays (x, y, z, field).
 template <typename T>
-__global__ void __launch_bounds__(SUB_NT, 1)
-k_substep(Layout L, Par<T> par, const T* __restrict__ P, const T* __restrict__ met, const T* __restrict__ Uin,
-          const T* __restrict__ U0, T* __restrict__ Uout, T* __restrict__ Pout, int stage, T dt,
-          unsigned long long* __restrict__ counters) {
+__global__ void __launch_bounds__(Tile<T>::NT, 1)
+k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmM, Layout L, Par<T> par,
+          const T* __restrict__ Uin, const T* __restrict__ U0, T* __restrict__ Uout, T* __restrict__ Pout, int stage,
+          T dt, unsigned long long* __restrict__ counters) {
   using G = TileGeom<T>;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* sF = reinterpret_cast<T*>(smem_raw);  // sF[q * NF + face]
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* sP = reinterpret_cast<T*>(smem_raw + G::OFF_P);  // sP[field][z][y][x], halo 2
+  T* sM = reinterpret_cast<T*>(smem_raw + G::OFF_M);  // sM[field][z][y][x], halo 1 (2 in x)
+  T* sF = reinterpret_cast<T*>(smem_raw + G::OFF_F);  // sF[q * NF + face]
+  const unsigned bar = smem_addr(smem_raw + G::OFF_BAR);
   const int x0 = blockIdx.x * G::TX, y0 = blockIdx.y * G::TY, z0 = blockIdx.z * G::TZ;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
+  // ---- stage-in: two TMA boxes, one mbarrier ----
+  if (threadIdx.x == 0) mbar_init(bar, 1);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    mbar_expect_tx(bar, G::TX_BYTES);
+    // storage coordinates of tile-local cell (-HX,-2,-2) / (-HX,-1,-1); out-of-range parts are zero-filled
+    tma_load_4d(smem_addr(sP), &tmP, bar, x0 + L.ox - G::HX, y0 + L.g[1] - NG, z0 + L.g[2] - NG, 0);
+    tma_load_4d(smem_addr(sM), &tmM, bar, x0 + L.ox - G::HX, y0 + L.g[1] - 1, z0 + L.g[2] - 1, 0);
+  }
+  // this thread's cell of phase 2 (one cell per thread) and its conserved inputs: the loads fly during phase 1
+  const int ca = threadIdx.x % G::TX, cr = threadIdx.x / G::TX;
+  const int cb = cr % G::TY, cc = cr / G::TY;
+  const int ci = x0 + ca, cj = y0 + cb, ck = z0 + cc;
+  const bool cell_ok = ci < L.n[0] && cj < L.n[1] && ck < L.n[2];
+  const long long id = L.idx(ci, cj, ck);
+  mbar_wait(bar, 0);
+
   // ---- phase 1: every face of the tile once ----
 #pragma unroll 1
-  for (int task = warp; task < G::WX + G::WY + G::WZ; task += SUB_NT / 32) {
+  for (int task = warp; task < G::WX + G::WY + G::WZ; task += G::NT / 32) {
     int d = (task >= G::WX) + (task >= G::WX + G::WY);
     // keep ONE copy of the face-flux body: hide the value of d so the compiler does not clone it per axis
     asm volatile("" : "+r"(d));
@@ -247,13 +361,15 @@ k_substep(Layout L, Par<T> par, const T* __restrict__ P, const T* __restrict__ m
     if (d == 0) { a = f % (G::TX + 1); const int r = f / (G::TX + 1); b = r % G::TY; c = r / G::TY; }
     else if (d == 1) { a = f % G::TX; const int r = f / G::TX; b = r % (G::TY + 1); c = r / (G::TY + 1); }
     else { a = f % G::TX; const int r = f / G::TX; b = r % G::TY; c = r / G::TY; }
-    const int gi = x0 + a, gj = y0 + b, gk = z0 + c;
-    // the face lies between cell (gi,gj,gk) - e_d and cell (gi,gj,gk)
-    const bool valid = gi < L.n[0] + (d == 0) && gj < L.n[1] + (d == 1) && gk < L.n[2] + (d == 2);
+    // the face lies between cell (a,b,c) - e_d and cell (a,b,c)
+    const bool valid = x0 + a < L.n[0] + (d == 0) && y0 + b < L.n[1] + (d == 1) && z0 + c < L.n[2] + (d == 2);
     if (!valid) continue;
-    const long long id = L.idx(gi, gj, gk) - L.stride(d);
+    const int sp = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::BY);
+    const int sm = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::MY);
+    const T* sPc = sP + ((c + NG) * G::BY + (b + NG)) * G::BX + (a + G::HX) - sp;
+    const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX) - sm;
     T Phi[NV];
-    face_flux_rot<T>(L, P, met, id, d, par, Phi);
+    face_flux_rot<T>(sPc, sMc, sp, sm, d, par, Phi);
     T* o = sF + off + f;
     o[0] = Phi[0];
     o[4 * G::NF] = Phi[4];
@@ -265,17 +381,22 @@ k_substep(Layout L, Par<T> par, const T* __restrict__ P, const T* __restrict__ m
       o[(5 + t) * G::NF] = Phi[5 + c3];
     }
   }
+  // conserved inputs of this thread's cell: issued before the barrier so their latency overlaps the wait
+  T u[NV], u0[NV];
+  if (cell_ok) {
+#pragma unroll
+    for (int v = 0; v < NV; v++) u[v] = Uin[v * L.fs + id];
+    if (stage != 0) {
+#pragma unroll
+      for (int v = 0; v < NV; v++) u0[v] = U0[v * L.fs + id];
+    }
+  }
   __syncthreads();
 
-  // ---- phase 2: per cell ----
+  // ---- phase 2: one cell per thread ----
   int fail = 0, reset = 0, pfl = 0, it = 0;
-#pragma unroll 1
-  for (int cidx = threadIdx.x; cidx < G::NC; cidx += SUB_NT) {
-    const int a = cidx % G::TX, r = cidx / G::TX;
-    const int b = r % G::TY, c = r / G::TY;
-    const int i = x0 + a, j = y0 + b, k = z0 + c;
-    if (i >= L.n[0] || j >= L.n[1] || k >= L.n[2]) continue;
-    const long long id = L.idx(i, j, k);
+  if (cell_ok) {
+    const int a = ca, b = cb, c = cc;
     T R[NV];
 #pragma unroll
     for (int q = 0; q < NV; q++) R[q] = 0;
@@ -297,30 +418,33 @@ k_substep(Layout L, Par<T> par, const T* __restrict__ P, const T* __restrict__ m
 #pragma unroll
       for (int q = 0; q < NV; q++) R[q] -= (o[q * G::NF + G::TX * G::TY] - o[q * G::NF]) * ih;
     }
-    T q[NV];
-    load_fields(P, L.fs, id, NV, q);
-    add_sources(L, met, id, q, par, R);
-    // a7: Runge-Kutta stage combine
-    T u[NV];
+    const T* sPc = sP + ((c + NG) * G::BY + (b + NG)) * G::BX + (a + G::HX);
+    const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX);
+    T q[NV], m[NM];
 #pragma unroll
-    for (int v = 0; v < NV; v++) {
-      T u1 = Uin[v * L.fs + id] + dt * R[v];
-      if (stage == 1) u1 = T(0.75) * U0[v * L.fs + id] + T(0.25) * u1;
-      if (stage == 2) u1 = T(1.0 / 3.0) * U0[v * L.fs + id] + T(2.0 / 3.0) * u1;
-      u[v] = u1;
-    }
-    // a8: primitive recovery and floors
-    T m[NM];
-    load_fields(met, L.fs, id, NM, m);
+    for (int v = 0; v < NV; v++) q[v] = sPc[v * G::PFS];
+#pragma unroll
+    for (int v = 0; v < NM; v++) m[v] = sMc[v * G::MFS];
     T cf[6], gi[6];
     const T det = cofactors(m + GXX, cf);
     const T sq = sqrt_(det);
     const T idet = rcp_(det);
 #pragma unroll
     for (int a6 = 0; a6 < 6; a6++) gi[a6] = cf[a6] * idet;
+    add_sources_staged(L, sMc, m, q, par, gi, sq, R);
+    // a7: Runge-Kutta stage combine
+#pragma unroll
+    for (int v = 0; v < NV; v++) {
+      T u1 = u[v] + dt * R[v];
+      if (stage == 1) u1 = T(0.75) * u0[v] + T(0.25) * u1;
+      if (stage == 2) u1 = T(1.0 / 3.0) * u0[v] + T(2.0 / 3.0) * u1;
+      u[v] = u1;
+    }
+    // a8: primitive recovery and floors
+    const T isq = rcp_(sq);
     T w[NV];
 #pragma unroll
-    for (int v = 0; v < NV; v++) w[v] = u[v] / sq;
+    for (int v = 0; v < NV; v++) w[v] = u[v] * isq;
     if (!par.cleaning) w[8] = 0;
     T Zg;
     {  // guess from the previous primitives of this cell
@@ -332,7 +456,7 @@ k_substep(Layout L, Par<T> par, const T* __restrict__ P, const T* __restrict__ m
     T qn[NV];
     int its = 0;
     const int fl = con2prim(w, m, gi, par, Zg, qn, its);
-    it = its > it ? its : it;
+    it = its;
     bool rs = fl != 0;
     if (!rs && qn[RHO] < par.rho_thr) rs = true;
     bool pf = false;
@@ -351,10 +475,10 @@ k_substep(Layout L, Par<T> par, const T* __restrict__ P, const T* __restrict__ m
 #pragma unroll
       for (int v = 0; v < NV; v++) u[v] = sq * un[v];
     }
-    fail += fl != 0; reset += rs; pfl += pf;
+    fail = fl != 0; reset = rs; pfl = pf;
 #pragma unroll
     for (int v = 0; v < NV; v++) Uout[v * L.fs + id] = u[v];
-    store_prims_with_images(L, Pout, i, j, k, qn);
+    store_prims_with_images(L, Pout, ci, cj, ck, qn);
   }
   // warp-level reduction of the counters: [0] c2p_fail, [1] atm_reset, [2] p_floor, [3] max iterations
   const unsigned full = 0xffffffffu;
