@@ -102,6 +102,7 @@ struct hz_ctx {
   int pcur;   // P[pcur] holds the current primitives
   int stage;  // next Runge-Kutta stage 0, 1, 2
   bool have_metric, have_prim;
+  int nsm;                  // multiprocessors of the device (grid of the persistent substep kernel)
   CUtensorMap tmP[2], tmM;  // TMA descriptors of the two primitive sets and of the metric (k_substep stage-in)
   long long launches;
   bool prof;                          // per-kernel event timing on (hz_profile)
@@ -245,11 +246,13 @@ int substep_t(hz_ctx* c, double dt) {
   T* Uout = st == 0 ? c->U<T>(1 - c->cur) : c->U<T>(c->cur);
   const T* U0 = st == 0 ? Uin : c->U<T>(c->u0);
   using G = TileGeom<T>;
-  const dim3 grid((L.n[0] + G::TX - 1) / G::TX, (L.n[1] + G::TY - 1) / G::TY, (L.n[2] + G::TZ - 1) / G::TZ);
+  const int ntx = (L.n[0] + G::TX - 1) / G::TX, nty = (L.n[1] + G::TY - 1) / G::TY, ntz = (L.n[2] + G::TZ - 1) / G::TZ;
+  const long long ntiles = (long long)ntx * nty * ntz;
+  const unsigned grid = (unsigned)(ntiles < c->nsm ? ntiles : c->nsm);  // persistent: one block per SM
   {
     ProfScope ps(c, K_SUBSTEP);
     k_substep<T><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, Uin, U0, Uout,
-                                                        c->P<T>(1 - c->pcur), st, (T)dt, c->counters());
+                                                        c->P<T>(1 - c->pcur), st, (T)dt, c->counters(), ntx, nty, (int)ntiles);
   }
   HZ_LAUNCHED(c);
   if (st == 0) { c->u0 = c->cur; c->cur = 1 - c->cur; }
@@ -411,6 +414,11 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
   c->have_metric = c->have_prim = false;
   c->launches = 0;
   c->prof = false;
+  {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->nsm < 1) c->nsm = 148;
+  }
   if (HZ_DISPATCH(c, make_maps_t, c) != HZ_OK) {
     if (c->own) cudaFree(c->base);
     delete c;

@@ -1,6 +1,7 @@
 // hz_substep.cuh -- one Runge-Kutta substep as ONE kernel (rows a1-a9 of DESIGN.md section 2).
 //
 // A block owns a tile of TX x TY x TZ cells.
+// Blocks are persistent (one per SM) and take tiles round-robin.
 //   Stage-in : one thread issues two TMA box loads (cp.async.bulk.tensor.4d): the 9 primitives of the
 //              tile with a 2-cell halo and the 10 metric components with a 1-cell halo (2 in x, so
 //              both boxes share the x origin) land in shared memory; everyone waits on one mbarrier.
@@ -51,8 +52,11 @@ struct TileGeom {
   static constexpr size_t OFF_P = 0;
   static constexpr size_t OFF_M = align128(OFF_P + (size_t)NV * PFS * sizeof(T));
   static constexpr size_t OFF_F = align128(OFF_M + (size_t)NM * MFS * sizeof(T));
-  static constexpr size_t OFF_BAR = align128(OFF_F + (size_t)NV * NF * sizeof(T));
+  static constexpr size_t OFF_R = align128(OFF_F + (size_t)NV * NF * sizeof(T));
+  static constexpr size_t OFF_BAR = align128(OFF_R + (size_t)(NV - 1) * NC * sizeof(T));  // mbarrier (8 B), work queue (4 B)
   static constexpr size_t SMEM = OFF_BAR + 16;
+  static_assert(SMEM <= 227 * 1024, "tile does not fit the 227 KB of shared memory a block may use");
+  static constexpr int NFACE_TASKS = WX + WY + WZ, NSRC_TASKS = NC / 32;  // phase-1 work items (one warp each)
   static constexpr unsigned TX_BYTES = (unsigned)((NV * PFS + NM * MFS) * sizeof(T));
 };
 
@@ -315,170 +319,241 @@ __device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __re
       }
 }
 
+// ---- the work items of phase 1 ----------------------------------------------------------------------
+// Face item: 32 consecutive faces of one direction -> Phi into sF.
+template <typename T>
+__device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, const T* sP, const T* sM, T* sF, int task,
+                                          int lane, int x0, int y0, int z0) {
+  using G = TileGeom<T>;
+  int d = (task >= G::WX) + (task >= G::WX + G::WY);
+  // keep ONE copy of the face-flux body: hide the value of d so the compiler does not clone it per axis
+  asm volatile("" : "+r"(d));
+  const int off = d == 0 ? 0 : (d == 1 ? G::NFX : G::NFX + G::NFY);
+  const int f = task * 32 - off + lane;
+  if (L.g[d] == 0) return;
+  int a, b, c;  // face coordinates inside the tile; divisions by compile-time constants only
+  if (d == 0) { a = f % (G::TX + 1); const int r = f / (G::TX + 1); b = r % G::TY; c = r / G::TY; }
+  else if (d == 1) { a = f % G::TX; const int r = f / G::TX; b = r % (G::TY + 1); c = r / (G::TY + 1); }
+  else { a = f % G::TX; const int r = f / G::TX; b = r % G::TY; c = r / G::TY; }
+  // the face lies between cell (a,b,c) - e_d and cell (a,b,c)
+  const bool valid = x0 + a < L.n[0] + (d == 0) && y0 + b < L.n[1] + (d == 1) && z0 + c < L.n[2] + (d == 2);
+  if (!valid) return;
+  const int sp = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::BY);
+  const int sm = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::MY);
+  const T* sPc = sP + ((c + NG) * G::BY + (b + NG)) * G::BX + (a + G::HX) - sp;
+  const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX) - sm;
+  T Phi[NV];
+  face_flux_rot<T>(sPc, sMc, sp, sm, d, par, Phi);
+  T* o = sF + off + f;
+  o[0] = Phi[0];
+  o[4 * G::NF] = Phi[4];
+  o[8 * G::NF] = Phi[8];
+#pragma unroll
+  for (int c3 = 0; c3 < 3; c3++) {
+    const int t = rot3(d, c3);
+    o[(1 + t) * G::NF] = Phi[1 + c3];
+    o[(5 + t) * G::NF] = Phi[5 + c3];
+  }
+}
+
+// Source item: the geometric and cleaning sources (a6) of 32 cells -> sR[(q-1) * NC + cell], q = 1..8
+// (the D equation has no source).  Needs no flux, so it fills the scheduling gaps of the face items.
+template <typename T>
+__device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, const T* sP, const T* sM, T* sR,
+                                            int cell, int x0, int y0, int z0) {
+  using G = TileGeom<T>;
+  const int a = cell % G::TX, r = cell / G::TX;
+  const int b = r % G::TY, c = r / G::TY;
+  if (x0 + a >= L.n[0] || y0 + b >= L.n[1] || z0 + c >= L.n[2]) return;
+  const T* sPc = sP + ((c + NG) * G::BY + (b + NG)) * G::BX + (a + G::HX);
+  const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX);
+  T q[NV], m[NM];
+#pragma unroll
+  for (int v = 0; v < NV; v++) q[v] = sPc[v * G::PFS];
+#pragma unroll
+  for (int v = 0; v < NM; v++) m[v] = sMc[v * G::MFS];
+  T cf[6], gi[6];
+  const T det = cofactors(m + GXX, cf);
+  const T sq = sqrt_(det);
+  const T idet = rcp_(det);
+#pragma unroll
+  for (int a6 = 0; a6 < 6; a6++) gi[a6] = cf[a6] * idet;
+  T R[NV];
+#pragma unroll
+  for (int v = 0; v < NV; v++) R[v] = 0;
+  add_sources_staged(L, sMc, m, q, par, gi, sq, R);
+#pragma unroll
+  for (int v = 1; v < NV; v++) sR[(v - 1) * G::NC + cell] = R[v];
+}
+
+// One thread: the two TMA boxes of `tile` (primitives, metric), completion on `bar`.
+template <typename T>
+__device__ __forceinline__ void issue_loads(const CUtensorMap* tmP, const CUtensorMap* tmM, const Layout& L, T* sP, T* sM,
+                                            unsigned bar, int tile, int ntx, int nty) {
+  using G = TileGeom<T>;
+  const int tx = tile % ntx, r = tile / ntx;
+  const int x0 = tx * G::TX, y0 = (r % nty) * G::TY, z0 = (r / nty) * G::TZ;
+  mbar_expect_tx(bar, G::TX_BYTES);
+  // storage coordinates of tile-local cell (-HX,-2,-2) / (-HX,-1,-1); out-of-range parts are zero-filled
+  tma_load_4d(smem_addr(sP), tmP, bar, x0 + L.ox - G::HX, y0 + L.g[1] - NG, z0 + L.g[2] - NG, 0);
+  tma_load_4d(smem_addr(sM), tmM, bar, x0 + L.ox - G::HX, y0 + L.g[1] - 1, z0 + L.g[2] - 1, 0);
+}
+
+// ---- the kernel: persistent blocks, one tile per iteration ----------------------------------------
 // stage 0: Uout = Uin + dt L;  1: Uout = 3/4 U0 + 1/4 (Uin + dt L);  2: Uout = 1/3 U0 + 2/3 (Uin + dt L)
 // tmP / tmM: tensor maps of the current primitives and of the metric as 4D arrays (x, y, z, field).
+// Tiles are numbered x fastest; block b takes tiles b, b + gridDim.x, ...  While a block is in phase 2
+// of one tile, the TMA loads of its next tile are already in flight (the staged boxes are dead by then).
 template <typename T>
 __global__ void __launch_bounds__(Tile<T>::NT, 1)
 k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmM, Layout L, Par<T> par,
           const T* __restrict__ Uin, const T* __restrict__ U0, T* __restrict__ Uout, T* __restrict__ Pout, int stage,
-          T dt, unsigned long long* __restrict__ counters) {
+          T dt, unsigned long long* __restrict__ counters, int ntx, int nty, int ntiles) {
   using G = TileGeom<T>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  T* sP = reinterpret_cast<T*>(smem_raw + G::OFF_P);  // sP[field][z][y][x], halo 2
-  T* sM = reinterpret_cast<T*>(smem_raw + G::OFF_M);  // sM[field][z][y][x], halo 1 (2 in x)
+  T* sP = reinterpret_cast<T*>(smem_raw + G::OFF_P);  // sP[field][z][y][x], halo 2 (HX in x)
+  T* sM = reinterpret_cast<T*>(smem_raw + G::OFF_M);  // sM[field][z][y][x], halo 1 (HX in x)
   T* sF = reinterpret_cast<T*>(smem_raw + G::OFF_F);  // sF[q * NF + face]
+  T* sR = reinterpret_cast<T*>(smem_raw + G::OFF_R);  // sR[(q-1) * NC + cell]
+  int* queue = reinterpret_cast<int*>(smem_raw + G::OFF_BAR + 8);
   const unsigned bar = smem_addr(smem_raw + G::OFF_BAR);
-  const int x0 = blockIdx.x * G::TX, y0 = blockIdx.y * G::TY, z0 = blockIdx.z * G::TZ;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
 
-  // ---- stage-in: two TMA boxes, one mbarrier ----
-  if (threadIdx.x == 0) mbar_init(bar, 1);
-  __syncthreads();
   if (threadIdx.x == 0) {
-    mbar_expect_tx(bar, G::TX_BYTES);
-    // storage coordinates of tile-local cell (-HX,-2,-2) / (-HX,-1,-1); out-of-range parts are zero-filled
-    tma_load_4d(smem_addr(sP), &tmP, bar, x0 + L.ox - G::HX, y0 + L.g[1] - NG, z0 + L.g[2] - NG, 0);
-    tma_load_4d(smem_addr(sM), &tmM, bar, x0 + L.ox - G::HX, y0 + L.g[1] - 1, z0 + L.g[2] - 1, 0);
+    mbar_init(bar, 1);
+    *queue = 0;
   }
-  // this thread's cell of phase 2 (one cell per thread) and its conserved inputs: the loads fly during phase 1
+  __syncthreads();
+  if (threadIdx.x == 0 && (int)blockIdx.x < ntiles) issue_loads<T>(&tmP, &tmM, L, sP, sM, bar, blockIdx.x, ntx, nty);
+
+  // this thread's cell of phase 2 (one cell per thread), tile-local
   const int ca = threadIdx.x % G::TX, cr = threadIdx.x / G::TX;
   const int cb = cr % G::TY, cc = cr / G::TY;
-  const int ci = x0 + ca, cj = y0 + cb, ck = z0 + cc;
-  const bool cell_ok = ci < L.n[0] && cj < L.n[1] && ck < L.n[2];
-  const long long id = L.idx(ci, cj, ck);
-  mbar_wait(bar, 0);
-
-  // ---- phase 1: every face of the tile once ----
-#pragma unroll 1
-  for (int task = warp; task < G::WX + G::WY + G::WZ; task += G::NT / 32) {
-    int d = (task >= G::WX) + (task >= G::WX + G::WY);
-    // keep ONE copy of the face-flux body: hide the value of d so the compiler does not clone it per axis
-    asm volatile("" : "+r"(d));
-    const int off = d == 0 ? 0 : (d == 1 ? G::NFX : G::NFX + G::NFY);
-    const int f = task * 32 - off + lane;
-    if (L.g[d] == 0) continue;
-    int a, b, c;  // face coordinates inside the tile; divisions by compile-time constants only
-    if (d == 0) { a = f % (G::TX + 1); const int r = f / (G::TX + 1); b = r % G::TY; c = r / G::TY; }
-    else if (d == 1) { a = f % G::TX; const int r = f / G::TX; b = r % (G::TY + 1); c = r / (G::TY + 1); }
-    else { a = f % G::TX; const int r = f / G::TX; b = r % G::TY; c = r / G::TY; }
-    // the face lies between cell (a,b,c) - e_d and cell (a,b,c)
-    const bool valid = x0 + a < L.n[0] + (d == 0) && y0 + b < L.n[1] + (d == 1) && z0 + c < L.n[2] + (d == 2);
-    if (!valid) continue;
-    const int sp = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::BY);
-    const int sm = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::MY);
-    const T* sPc = sP + ((c + NG) * G::BY + (b + NG)) * G::BX + (a + G::HX) - sp;
-    const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX) - sm;
-    T Phi[NV];
-    face_flux_rot<T>(sPc, sMc, sp, sm, d, par, Phi);
-    T* o = sF + off + f;
-    o[0] = Phi[0];
-    o[4 * G::NF] = Phi[4];
-    o[8 * G::NF] = Phi[8];
-#pragma unroll
-    for (int c3 = 0; c3 < 3; c3++) {
-      const int t = rot3(d, c3);
-      o[(1 + t) * G::NF] = Phi[1 + c3];
-      o[(5 + t) * G::NF] = Phi[5 + c3];
-    }
-  }
-  // conserved inputs of this thread's cell: issued before the barrier so their latency overlaps the wait
-  T u[NV], u0[NV];
-  if (cell_ok) {
-#pragma unroll
-    for (int v = 0; v < NV; v++) u[v] = Uin[v * L.fs + id];
-    if (stage != 0) {
-#pragma unroll
-      for (int v = 0; v < NV; v++) u0[v] = U0[v * L.fs + id];
-    }
-  }
-  __syncthreads();
-
-  // ---- phase 2: one cell per thread ----
+  const T* sPc = sP + ((cc + NG) * G::BY + (cb + NG)) * G::BX + (ca + G::HX);
+  const T* sMc = sM + ((cc + 1) * G::MY + (cb + 1)) * G::BX + (ca + G::HX);
   int fail = 0, reset = 0, pfl = 0, it = 0;
-  if (cell_ok) {
-    const int a = ca, b = cb, c = cc;
-    T R[NV];
-#pragma unroll
-    for (int q = 0; q < NV; q++) R[q] = 0;
-    if (L.g[0]) {
-      const T ih = T(1.0 / L.h[0]);
-      const T* o = sF + (c * G::TY + b) * (G::TX + 1) + a;
-#pragma unroll
-      for (int q = 0; q < NV; q++) R[q] -= (o[q * G::NF + 1] - o[q * G::NF]) * ih;
+  unsigned parity = 0;
+
+#pragma unroll 1
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, parity ^= 1u) {
+    const int tx = tile % ntx, tr = tile / ntx;
+    const int x0 = tx * G::TX, y0 = (tr % nty) * G::TY, z0 = (tr / nty) * G::TZ;
+    const int ci = x0 + ca, cj = y0 + cb, ck = z0 + cc;
+    const bool cell_ok = ci < L.n[0] && cj < L.n[1] && ck < L.n[2];
+    const long long id = L.idx(ci, cj, ck);
+    mbar_wait(bar, parity);
+
+    // ---- phase 1: work queue of face items, then source items ----
+#pragma unroll 1
+    for (;;) {
+      int t = 0;
+      if (lane == 0) t = atomicAdd(queue, 1);
+      t = __shfl_sync(0xffffffffu, t, 0);
+      if (t >= G::NFACE_TASKS + G::NSRC_TASKS) break;
+      if (t < G::NFACE_TASKS) face_task<T>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
+      else source_task<T>(L, par, sP, sM, sR, (t - G::NFACE_TASKS) * 32 + lane, x0, y0, z0);
     }
-    if (L.g[1]) {
-      const T ih = T(1.0 / L.h[1]);
-      const T* o = sF + G::NFX + (c * (G::TY + 1) + b) * G::TX + a;
+    // inputs of this thread's cell: conserved state from HBM (latency overlaps the barrier wait),
+    // previous primitives and metric from the staged boxes (free for the next tile afterwards)
+    T u[NV], u0[NV], q[NV], m[NM];
+    if (cell_ok) {
 #pragma unroll
-      for (int q = 0; q < NV; q++) R[q] -= (o[q * G::NF + G::TX] - o[q * G::NF]) * ih;
-    }
-    if (L.g[2]) {
-      const T ih = T(1.0 / L.h[2]);
-      const T* o = sF + G::NFX + G::NFY + (c * G::TY + b) * G::TX + a;
+      for (int v = 0; v < NV; v++) u[v] = Uin[v * L.fs + id];
+      if (stage != 0) {
 #pragma unroll
-      for (int q = 0; q < NV; q++) R[q] -= (o[q * G::NF + G::TX * G::TY] - o[q * G::NF]) * ih;
+        for (int v = 0; v < NV; v++) u0[v] = U0[v * L.fs + id];
+      }
     }
-    const T* sPc = sP + ((c + NG) * G::BY + (b + NG)) * G::BX + (a + G::HX);
-    const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX);
-    T q[NV], m[NM];
 #pragma unroll
     for (int v = 0; v < NV; v++) q[v] = sPc[v * G::PFS];
 #pragma unroll
     for (int v = 0; v < NM; v++) m[v] = sMc[v * G::MFS];
-    T cf[6], gi[6];
-    const T det = cofactors(m + GXX, cf);
-    const T sq = sqrt_(det);
-    const T idet = rcp_(det);
-#pragma unroll
-    for (int a6 = 0; a6 < 6; a6++) gi[a6] = cf[a6] * idet;
-    add_sources_staged(L, sMc, m, q, par, gi, sq, R);
-    // a7: Runge-Kutta stage combine
-#pragma unroll
-    for (int v = 0; v < NV; v++) {
-      T u1 = u[v] + dt * R[v];
-      if (stage == 1) u1 = T(0.75) * u0[v] + T(0.25) * u1;
-      if (stage == 2) u1 = T(1.0 / 3.0) * u0[v] + T(2.0 / 3.0) * u1;
-      u[v] = u1;
+    __syncthreads();  // all fluxes and sources are in shared memory; nobody reads sP / sM any more
+    if (threadIdx.x == 0) {
+      *queue = 0;
+      if (tile + (int)gridDim.x < ntiles) issue_loads<T>(&tmP, &tmM, L, sP, sM, bar, tile + gridDim.x, ntx, nty);
     }
-    // a8: primitive recovery and floors
-    const T isq = rcp_(sq);
-    T w[NV];
+
+    // ---- phase 2: one cell per thread ----
+    if (cell_ok) {
+      T R[NV];
+      R[0] = 0;
 #pragma unroll
-    for (int v = 0; v < NV; v++) w[v] = u[v] * isq;
-    if (!par.cleaning) w[8] = 0;
-    T Zg;
-    {  // guess from the previous primitives of this cell
-      T utl[3];
-      lower(m + GXX, q + UX, utl);
-      const T W2 = 1 + dot3(q + UX, utl);
-      Zg = (q[RHO] + par.gg1 * q[PR]) * W2;
+      for (int v = 1; v < NV; v++) R[v] = sR[(v - 1) * G::NC + threadIdx.x];
+      if (L.g[0]) {
+        const T ih = T(1.0 / L.h[0]);
+        const T* o = sF + (cc * G::TY + cb) * (G::TX + 1) + ca;
+#pragma unroll
+        for (int v = 0; v < NV; v++) R[v] -= (o[v * G::NF + 1] - o[v * G::NF]) * ih;
+      }
+      if (L.g[1]) {
+        const T ih = T(1.0 / L.h[1]);
+        const T* o = sF + G::NFX + (cc * (G::TY + 1) + cb) * G::TX + ca;
+#pragma unroll
+        for (int v = 0; v < NV; v++) R[v] -= (o[v * G::NF + G::TX] - o[v * G::NF]) * ih;
+      }
+      if (L.g[2]) {
+        const T ih = T(1.0 / L.h[2]);
+        const T* o = sF + G::NFX + G::NFY + (cc * G::TY + cb) * G::TX + ca;
+#pragma unroll
+        for (int v = 0; v < NV; v++) R[v] -= (o[v * G::NF + G::TX * G::TY] - o[v * G::NF]) * ih;
+      }
+      if (!par.cleaning) R[8] = 0;
+      // a7: Runge-Kutta stage combine
+#pragma unroll
+      for (int v = 0; v < NV; v++) {
+        T u1 = u[v] + dt * R[v];
+        if (stage == 1) u1 = T(0.75) * u0[v] + T(0.25) * u1;
+        if (stage == 2) u1 = T(1.0 / 3.0) * u0[v] + T(2.0 / 3.0) * u1;
+        u[v] = u1;
+      }
+      // a8: primitive recovery and floors
+      T cf[6], gi[6];
+      const T det = cofactors(m + GXX, cf);
+      const T sq = sqrt_(det);
+      const T idet = rcp_(det);
+#pragma unroll
+      for (int a6 = 0; a6 < 6; a6++) gi[a6] = cf[a6] * idet;
+      const T isq = rcp_(sq);
+      T w[NV];
+#pragma unroll
+      for (int v = 0; v < NV; v++) w[v] = u[v] * isq;
+      if (!par.cleaning) w[8] = 0;
+      T Zg;
+      {  // guess from the previous primitives of this cell
+        T utl[3];
+        lower(m + GXX, q + UX, utl);
+        const T W2 = 1 + dot3(q + UX, utl);
+        Zg = (q[RHO] + par.gg1 * q[PR]) * W2;
+      }
+      T qn[NV];
+      int its = 0;
+      const int fl = con2prim(w, m, gi, par, Zg, qn, its);
+      it = its > it ? its : it;
+      bool rs = fl != 0;
+      if (!rs && qn[RHO] < par.rho_thr) rs = true;
+      bool pf = false;
+      if (rs) {
+        qn[RHO] = par.rho_atm; qn[PR] = par.p_atm;
+#pragma unroll
+        for (int a3 = 0; a3 < 3; a3++) { qn[UX + a3] = 0; qn[BX + a3] = w[5 + a3]; }
+        qn[PSI] = w[8];
+      } else if (qn[PR] < par.p_atm) {
+        pf = true;
+        qn[PR] = par.p_atm;
+      }
+      if (rs || pf) {
+        T un[NV];
+        prim2con(qn, m, par, un);
+#pragma unroll
+        for (int v = 0; v < NV; v++) u[v] = sq * un[v];
+      }
+      fail += fl != 0; reset += rs; pfl += pf;
+#pragma unroll
+      for (int v = 0; v < NV; v++) Uout[v * L.fs + id] = u[v];
+      store_prims_with_images(L, Pout, ci, cj, ck, qn);
     }
-    T qn[NV];
-    int its = 0;
-    const int fl = con2prim(w, m, gi, par, Zg, qn, its);
-    it = its;
-    bool rs = fl != 0;
-    if (!rs && qn[RHO] < par.rho_thr) rs = true;
-    bool pf = false;
-    if (rs) {
-      qn[RHO] = par.rho_atm; qn[PR] = par.p_atm;
-#pragma unroll
-      for (int a3 = 0; a3 < 3; a3++) { qn[UX + a3] = 0; qn[BX + a3] = w[5 + a3]; }
-      qn[PSI] = w[8];
-    } else if (qn[PR] < par.p_atm) {
-      pf = true;
-      qn[PR] = par.p_atm;
-    }
-    if (rs || pf) {
-      T un[NV];
-      prim2con(qn, m, par, un);
-#pragma unroll
-      for (int v = 0; v < NV; v++) u[v] = sq * un[v];
-    }
-    fail = fl != 0; reset = rs; pfl = pf;
-#pragma unroll
-    for (int v = 0; v < NV; v++) Uout[v * L.fs + id] = u[v];
-    store_prims_with_images(L, Pout, ci, cj, ck, qn);
+    __syncthreads();  // sF / sR may be overwritten by the next tile's phase 1
   }
   // warp-level reduction of the counters: [0] c2p_fail, [1] atm_reset, [2] p_floor, [3] max iterations
   const unsigned full = 0xffffffffu;
