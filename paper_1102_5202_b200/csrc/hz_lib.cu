@@ -135,6 +135,7 @@ Par<T> make_par(const hz_ctx* c) {
   p.c2p_tol = (T)(h.c2p_tol > 0 ? h.c2p_tol : (sizeof(T) == 8 ? 1e-13 : 1e-6));
   p.c2p_maxit = h.c2p_maxit;
   p.cleaning = h.cleaning;
+  for (int d = 0; d < 3; d++) p.ih[d] = (T)(1.0 / c->L.h[d]);
   return p;
 }
 

@@ -25,22 +25,59 @@ struct Par {
   T rho_thr;   // rho_atm*(1+atm_tol)
   T kappa;
   T c2p_tol;
+  T ih[3];     // 1/dx, 1/dy, 1/dz
   int c2p_maxit;
   int cleaning;
 };
 
 // ---- scalar helpers -----------------------------------------------------------------------------
+// Reciprocal, division and square roots without the library's special-case branches: every operand
+// on this path is a normal, finite, positive-scale number (densities, determinants, 1 - v^2 a^2 ...).
+// fp64: hardware seed (MUFU.RCP64H, ~20 bits) + one cubic Newton step (error ~2^-60) and, for the
+// quotient, one residual correction; results agree with IEEE division to the last bit or two.
+// fp32: the hardware approximations (1-2 ulp), far inside the fp32 parity tolerance.
+__device__ __forceinline__ double rcp_(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x, y, 1.0);
+  const double e2 = fma(e, e, e);
+  return fma(y, e2, y);
+}
+__device__ __forceinline__ float rcp_(float x) {
+  float y;
+  asm("rcp.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ double div_(double a, double b) {
+  const double y = rcp_(b);
+  const double q = a * y;
+  const double r = fma(-b, q, a);
+  return fma(y, r, q);
+}
+__device__ __forceinline__ float div_(float a, float b) {
+  float q;
+  asm("div.approx.f32 %0, %1, %2;" : "=f"(q) : "f"(a), "f"(b));
+  return q;
+}
 __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
-__device__ __forceinline__ float sqrt_(float x) { return sqrtf(x); }
+__device__ __forceinline__ float sqrt_(float x) {
+  float y;
+  asm("sqrt.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ double rsqrt_(double x) { return rsqrt(x); }
-__device__ __forceinline__ float rsqrt_(float x) { return rsqrtf(x); }
-__device__ __forceinline__ double rcp_(double x) { return 1.0 / x; }
-__device__ __forceinline__ float rcp_(float x) { return 1.0f / x; }
+__device__ __forceinline__ float rsqrt_(float x) {
+  float y;
+  asm("rsqrt.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ double abs_(double x) { return fabs(x); }
 __device__ __forceinline__ float abs_(float x) { return fabsf(x); }
-__device__ __forceinline__ double min_(double a, double b) { return fmin(a, b); }
+// fp64 min/max as one compare and a select (no NaN fix-up: operands here are never NaN by construction,
+// and a NaN state is caught by the finite checks of the primitive recovery)
+__device__ __forceinline__ double min_(double a, double b) { return a < b ? a : b; }
 __device__ __forceinline__ float min_(float a, float b) { return fminf(a, b); }
-__device__ __forceinline__ double max_(double a, double b) { return fmax(a, b); }
+__device__ __forceinline__ double max_(double a, double b) { return a > b ? a : b; }
 __device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
 __device__ __forceinline__ bool finite_(double x) { return isfinite(x); }
 __device__ __forceinline__ bool finite_(float x) { return isfinite(x); }
@@ -105,7 +142,7 @@ __device__ __forceinline__ void eval_state(const T* q, const T* m, const Par<T>&
 #pragma unroll
   for (int i = 0; i < 3; i++) { s.v[i] = q[UX + i] * s.iW; s.vl[i] = utl[i] * s.iW; }
   s.v2 = ut2 * s.iW * s.iW;
-  s.rhoh = q[RHO] * (1 + par.gg1 * q[PR] / q[RHO]);
+  s.rhoh = q[RHO] + par.gg1 * q[PR];
   lower(m + GXX, q + BX, s.Bl);
   s.B2 = dot3(q + BX, s.Bl);
   s.Bv = dot3(q + BX, s.vl);
@@ -158,14 +195,14 @@ __device__ __forceinline__ void flux_speeds(const T* q, const T* m, const T* gid
     F[8] = 0;
   }
   // one fast-speed bound through the relativistic addition formula (R7)
-  T cs2 = par.Gam * q[PR] / s.rhoh;
-  T vA2 = s.b2 / (s.rhoh + s.b2);
+  T cs2 = div_(par.Gam * q[PR], s.rhoh);
+  T vA2 = div_(s.b2, s.rhoh + s.b2);
   T a2 = cs2 + vA2 - cs2 * vA2;
   a2 = min_(max_(a2, T(0)), T(1));
   T den = 1 - s.v2 * a2;
   T disc = a2 * (1 - s.v2) * (den * gid[D] - (1 - a2) * s.v[D] * s.v[D]);
   T sq = sqrt_(max_(disc, T(0)));
-  T aod = al / den;
+  T aod = div_(al, den);
   T vd = s.v[D] * (1 - a2);
   lp = aod * (vd + sq) - be;
   lm = aod * (vd - sq) - be;
@@ -196,7 +233,7 @@ __device__ __forceinline__ void hlle_face(T* qL, T* qR, const T* mf, const Par<T
   const T lm = min_(T(0), min_(lmL, lmR));
   const T w = lp - lm;
   if (w > T(1e-30)) {
-    const T sw = sq / w, ll = lp * lm;
+    const T sw = div_(sq, w), ll = lp * lm;
 #pragma unroll
     for (int q = 0; q < NV; q++) Phi[q] = sw * (lp * FL[q] - lm * FR[q] + ll * (UR[q] - UL[q]));
   } else {
@@ -288,7 +325,7 @@ __device__ __forceinline__ void c2p_eval(T Z, const C2P<T>& c, const Par<T>& par
   const T p = par.g1g * (Z * omv - c.D * sq);
   f = Z - p + c.B2 * (1 + v2) * T(0.5) - SB2 * T(0.5) * iZ2 - c.E;
   const T dv2 = -2 * (c.S2 * Z2 * Z + SB2 * (3 * Z2 + 3 * Z * c.B2 + c.B2 * c.B2)) * (iZ2 * iZ) * (iZB2 * iZB);
-  df = 1 - par.g1g * omv - par.g1g * (-Z + c.D / (2 * sq)) * dv2 + c.B2 * dv2 * T(0.5) + SB2 * iZ2 * iZ;
+  df = 1 - par.g1g * omv - par.g1g * (-Z + div_(c.D, 2 * sq)) * dv2 + c.B2 * dv2 * T(0.5) + SB2 * iZ2 * iZ;
 }
 
 // w: undensitised conserved; gi: inverse 3-metric (packed); Zg: guess.  Returns 0 on success.
@@ -319,7 +356,7 @@ __device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, con
   bool ok = false;
   for (int it = 1; it <= par.c2p_maxit; it++) {
     iters = it;
-    T Zn = Z - f / df;
+    T Zn = Z - div_(f, df);
     T v2n, fn, dfn;
     int halv = 0;
     for (;;) {  // keep Z > 0 and v^2 < 1 by halving the step
@@ -343,7 +380,7 @@ __device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, con
   q[RHO] = c.D * sq;
   q[PR] = par.g1g * (Z * omv - c.D * sq);
   const T iZB = rcp_(Z + c.B2);
-  const T sbz = c.SB / Z * iZB;
+  const T sbz = div_(c.SB, Z) * iZB;
 #pragma unroll
   for (int i = 0; i < 3; i++) {
     q[UX + i] = W * (Su[i] * iZB + sbz * w[5 + i]);

@@ -158,12 +158,12 @@ __device__ __forceinline__ void state_flux0(const T* q, const T* m, const T* gi0
     F[8] = 0;
   }
   // fast-speed bound a^2 = c_s^2 + v_A^2 - c_s^2 v_A^2 = (Gamma p + b^2)/(rho h + b^2)   (R7)
-  T a2 = (par.Gam * q[PR] + b2) / (rhoh + b2);
+  T a2 = div_(par.Gam * q[PR] + b2, rhoh + b2);
   a2 = min_(max_(a2, T(0)), T(1));
   const T den = 1 - v2 * a2;
   const T disc = a2 * (1 - v2) * (den * gi0[0] - (1 - a2) * v0 * v0);
   const T sq = sqrt_(max_(disc, T(0)));
-  const T aod = al / den;
+  const T aod = div_(al, den);
   const T vd = v0 * (1 - a2);
   lp = aod * (vd + sq) - be;
   lm = aod * (vd - sq) - be;
@@ -224,7 +224,7 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
   lm = min_(lm, T(0));
   const T w = lp - lm;
   if (w > T(1e-30)) {
-    const T sw = sqg / w, ll = lp * lm;
+    const T sw = div_(sqg, w), ll = lp * lm;
 #pragma unroll
     for (int q = 0; q < NV; q++) Phi[q] = sw * (lp * FL[q] - lm * FR[q] + ll * (UR[q] - UL[q]));
   } else {
@@ -251,7 +251,7 @@ __device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __r
       continue;
     }
     const int s = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::MY);
-    const T i2h = T(1.0 / (2 * L.h[d]));
+    const T i2h = T(0.5) * par.ih[d];
     T mp[NM], mm[NM];
 #pragma unroll
     for (int a = 0; a < NM; a++) { mp[a] = sMc[a * G::MFS + s]; mm[a] = sMc[a * G::MFS - s]; }
@@ -261,7 +261,7 @@ __device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __r
       T cp[6], cm[6];
       const T dp = cofactors(mp + GXX, cp), dn = cofactors(mm + GXX, cm);
       const T sp = sqrt_(dp), sn = sqrt_(dn);
-      const T ap = mp[AL] / sp, am = mm[AL] / sn;  // alpha sqrt(gamma) gamma^{kd} = alpha cof_kd / sqrt(gamma)
+      const T ap = div_(mp[AL], sp), am = div_(mm[AL], sn);  // alpha sqrt(gamma) gamma^{kd} = alpha cof_kd / sqrt(gamma)
 #pragma unroll
       for (int k = 0; k < 3; k++) dQ[k] += (ap * cp[sym(k, d)] - am * cm[sym(k, d)]) * i2h;
       dRb += (sp * mp[BEX + d] - sn * mm[BEX + d]) * i2h;
@@ -481,19 +481,19 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
 #pragma unroll
       for (int v = 1; v < NV; v++) R[v] = sR[(v - 1) * G::NC + threadIdx.x];
       if (L.g[0]) {
-        const T ih = T(1.0 / L.h[0]);
+        const T ih = par.ih[0];
         const T* o = sF + (cc * G::TY + cb) * (G::TX + 1) + ca;
 #pragma unroll
         for (int v = 0; v < NV; v++) R[v] -= (o[v * G::NF + 1] - o[v * G::NF]) * ih;
       }
       if (L.g[1]) {
-        const T ih = T(1.0 / L.h[1]);
+        const T ih = par.ih[1];
         const T* o = sF + G::NFX + (cc * (G::TY + 1) + cb) * G::TX + ca;
 #pragma unroll
         for (int v = 0; v < NV; v++) R[v] -= (o[v * G::NF + G::TX] - o[v * G::NF]) * ih;
       }
       if (L.g[2]) {
-        const T ih = T(1.0 / L.h[2]);
+        const T ih = par.ih[2];
         const T* o = sF + G::NFX + G::NFY + (cc * G::TY + cb) * G::TX + ca;
 #pragma unroll
         for (int v = 0; v < NV; v++) R[v] -= (o[v * G::NF + G::TX * G::TY] - o[v * G::NF]) * ih;
