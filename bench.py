@@ -32,13 +32,15 @@ SUBSTEPS_PER_STEP = 3
 # Algorithmic words per zone per substep of each kernel, cleaning on.
 # whole path: read P(9) + metric(10) + U^(k)(9) + U^n(9, stages 1-2 only -> 6 on average), write U(9) + P(9)
 ALGO_WORDS_PATH = 52.0
-# per kernel: what that launch must read and write if nothing is re-read
-KERNEL_WORDS = {
-    "k_rhs_update": 43.0,   # read P 9, metric 10, U^(k) 9, U^n 6 (stages 1-2); write U 9
-    "k_con2prim": 37.0,     # read U 9, metric 10, previous P 9 (guess); write P 9
-    "k_substep": 52.0,      # the fused whole-path kernel
-}
-ALGO_FLOPS_PATH = 3100.0   # survey estimate of the flops per zone-substep; DESIGN.md section 5
+# Algorithmic flops per zone per substep (executed fp64 flops of k_substep from ncu,
+# 4366, less the ~10 % that is duplicated tile-boundary face work; the plain oracle counts 4564 add+mul,
+# 648 div, 59 sqrt).  FMA = 2.
+ALGO_FLOPS_PATH = 3900.0
+# ALU peak (B200_PROFILING.md unit counts): 148 SMs x lanes x 2 flop x max SM clock
+SMS, LANES = 148, {"f64": 64, "f32": 128}
+# ncu dram__bytes_read.sum + dram__bytes_write.sum of one k_substep launch at 128^3, per zone
+# (profiles/r01_substep.md); scaled to the launch's zones below
+TRAFFIC_BYTES_PER_ZONE = {"f64": 495.0, "f32": 267.0}
 
 
 def peaks():
@@ -145,6 +147,17 @@ def run_reference(args):
     return 0
 
 
+def max_over_ranks(ms, world, device):
+    """Slowest rank's time: the only cross-rank operation of the replica path."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def run_gpu(args):
     import numpy as np
     import torch
@@ -199,10 +212,7 @@ def run_gpu(args):
     hz.profile(False)
     launches = hz.launch_count() - launches0
     clocks = sampler.stop(t0, t1) if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, "cuda")
     value = world * ncell * SUBSTEPS_PER_STEP * K / (ms * 1e-3)
     d = hz.diagnostics()
     finite = all(np.isfinite(v) for v in d.values())
@@ -226,10 +236,7 @@ def run_gpu(args):
     e1.record(stream)
     barrier()
     ms_e = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms_e], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e = float(t.item())
+    ms_e = max_over_ranks(ms_e, world, "cuda")
     e2e_value = world * ncell * SUBSTEPS_PER_STEP * Ke / (ms_e * 1e-3)
     assert bool(torch.isfinite(h_out).all()), "non-finite primitives after the end-to-end steps"
 
@@ -239,22 +246,28 @@ def run_gpu(args):
         return 0
 
     # ---- roofline of the dominant kernel ------------------------------------
+    # The path is bound by plain ALU arithmetic in both precisions (ALU bound 9.5 / 19 G zone-updates/s
+    # against 15.7 / 31.4 G for HBM), so the roofline is "alu"; the HBM view is reported beside it.
     hbm_gbs, peak_src, sm_max = peaks()
     tot_ms = sum(v[0] for v in prof.values())
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_n = prof[dom]
-    kw = KERNEL_WORDS.get(dom, ALGO_WORDS_PATH)
-    bytes_per_launch = kw * es * ncell
     avg_s = dom_ms * 1e-3 / max(dom_n, 1)
-    achieved = bytes_per_launch / avg_s / 1e9
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": achieved / hbm_gbs, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": avg_s * 1e3,
-                "share_of_step": dom_ms / tot_ms if tot_ms > 0 else None,
+    flops_per_launch = ALGO_FLOPS_PATH * ncell
+    bytes_per_launch = ALGO_WORDS_PATH * es * ncell
+    alu_peak = SMS * LANES[dtype] * 2 * sm_max * 1e6 / 1e12      # TFLOP/s
+    achieved = flops_per_launch / avg_s / 1e12
+    hbm_achieved = bytes_per_launch / avg_s / 1e9
+    roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
+                "frac": achieved / alu_peak,
+                "traffic": TRAFFIC_BYTES_PER_ZONE[dtype] * ncell,
+                "peak_source": f"derived: {SMS} SMs x {LANES[dtype]} {dtype} lanes x 2 x {sm_max:.0f} MHz (DESIGN.md section 5)",
+                "algorithmic_flops_per_launch": flops_per_launch, "algorithmic_bytes_per_launch": bytes_per_launch,
+                "avg_launch_ms": avg_s * 1e3, "share_of_step": dom_ms / tot_ms if tot_ms > 0 else None,
                 "kernels_ms_per_substep": {k: v[0] / (K * SUBSTEPS_PER_STEP) for k, v in prof.items() if v[1]},
-                # whole path against the two candidate bounds (north_star: the slower of the two)
-                "path_hbm_bound_zups": hbm_gbs * 1e9 / (ALGO_WORDS_PATH * es),
-                "path_frac_of_hbm_bound": (value / world) / (hbm_gbs * 1e9 / (ALGO_WORDS_PATH * es))}
+                "hbm_achieved_gbs": hbm_achieved, "hbm_peak_gbs": hbm_gbs, "hbm_frac": hbm_achieved / hbm_gbs,
+                "hbm_peak_source": peak_src,
+                "traffic_source": "ncu dram bytes of one launch at 128^3, per zone (profiles/r01_substep.md)"}
 
     # ---- the oracle on the host cores, bounded sample ---------------------------------------------
     cpu = None
