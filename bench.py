@@ -32,15 +32,15 @@ SUBSTEPS_PER_STEP = 3
 # Algorithmic words per zone per substep of each kernel, cleaning on.
 # whole path: read P(9) + metric(10) + U^(k)(9) + U^n(9, stages 1-2 only -> 6 on average), write U(9) + P(9)
 ALGO_WORDS_PATH = 52.0
-# Algorithmic flops per zone per substep (executed fp64 flops of k_substep from ncu,
-# 4366, less the ~10 % that is duplicated tile-boundary face work; the plain oracle counts 4564 add+mul,
-# 648 div, 59 sqrt).  FMA = 2.
-ALGO_FLOPS_PATH = 3900.0
+# Algorithmic flops per zone per substep (flops k_substep executes per zone by ncu,
+# 4120 in fp64 and 3190 in fp32, less the ~10 % that is duplicated tile-boundary face work; the plain
+# oracle counts 4564 add+mul, 648 div, 59 sqrt).  FMA = 2.
+ALGO_FLOPS = {"f64": 3700.0, "f32": 2900.0}
 # ALU peak (B200_PROFILING.md unit counts): 148 SMs x lanes x 2 flop x max SM clock
 SMS, LANES = 148, {"f64": 64, "f32": 128}
 # ncu dram__bytes_read.sum + dram__bytes_write.sum of one k_substep launch at 128^3, per zone
 # (profiles/r01_substep.md); scaled to the launch's zones below
-TRAFFIC_BYTES_PER_ZONE = {"f64": 495.0, "f32": 267.0}
+TRAFFIC_BYTES_PER_ZONE = {"f64": 497.0, "f32": 268.0}
 
 
 def peaks():
@@ -246,14 +246,14 @@ def run_gpu(args):
         return 0
 
     # ---- roofline of the dominant kernel ------------------------------------
-    # The path is bound by plain ALU arithmetic in both precisions (ALU bound 9.5 / 19 G zone-updates/s
+    # The path is bound by plain ALU arithmetic in both precisions (ALU bound 10.1 / 25.7 G zone-updates/s
     # against 15.7 / 31.4 G for HBM), so the roofline is "alu"; the HBM view is reported beside it.
     hbm_gbs, peak_src, sm_max = peaks()
     tot_ms = sum(v[0] for v in prof.values())
     dom = max(prof, key=lambda k: prof[k][0])
     dom_ms, dom_n = prof[dom]
     avg_s = dom_ms * 1e-3 / max(dom_n, 1)
-    flops_per_launch = ALGO_FLOPS_PATH * ncell
+    flops_per_launch = ALGO_FLOPS[dtype] * ncell
     bytes_per_launch = ALGO_WORDS_PATH * es * ncell
     alu_peak = SMS * LANES[dtype] * 2 * sm_max * 1e6 / 1e12      # TFLOP/s
     achieved = flops_per_launch / avg_s / 1e12
