@@ -319,6 +319,20 @@ __device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __re
       }
 }
 
+// n / N for 0 <= n < NMAX and a compile-time N: shift or multiply-shift, never a division
+template <int N, int NMAX>
+__device__ __forceinline__ int cdiv(int n) {
+  if ((N & (N - 1)) == 0) {
+    int sh = 0;
+    while ((1 << sh) < N) sh++;
+    return n >> sh;
+  }
+  constexpr unsigned M = 65536 / N + 1;
+  static_assert((long long)NMAX * ((long long)M * N - 65536) < 65536 && (long long)NMAX * M < (1ll << 32),
+                "cdiv: multiply-shift not exact on this range");
+  return (int)(((unsigned)n * M) >> 16);
+}
+
 // ---- the work items of phase 1 ----------------------------------------------------------------------
 // Face item: 32 consecutive faces of one direction -> Phi into sF.
 template <typename T>
@@ -331,10 +345,13 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
   const int off = d == 0 ? 0 : (d == 1 ? G::NFX : G::NFX + G::NFY);
   const int f = task * 32 - off + lane;
   if (L.g[d] == 0) return;
-  int a, b, c;  // face coordinates inside the tile; divisions by compile-time constants only
-  if (d == 0) { a = f % (G::TX + 1); const int r = f / (G::TX + 1); b = r % G::TY; c = r / G::TY; }
-  else if (d == 1) { a = f % G::TX; const int r = f / G::TX; b = r % (G::TY + 1); c = r / (G::TY + 1); }
-  else { a = f % G::TX; const int r = f / G::TX; b = r % G::TY; c = r / G::TY; }
+  // face coordinates inside the tile: f = (c * e1 + b) * e0 + a with e0 = TX (+1 for x faces),
+  // e1 = TY (+1 for y faces); the quotients by multiply-shift (d is a run-time value here)
+  const int e0 = G::TX + (d == 0), e1 = G::TY + (d == 1);
+  const int r = d == 0 ? cdiv<G::TX + 1, G::NF>(f) : cdiv<G::TX, G::NF>(f);
+  const int a = f - r * e0;
+  const int c = d == 1 ? cdiv<G::TY + 1, G::NF>(r) : cdiv<G::TY, G::NF>(r);
+  const int b = r - c * e1;
   // the face lies between cell (a,b,c) - e_d and cell (a,b,c)
   const bool valid = x0 + a < L.n[0] + (d == 0) && y0 + b < L.n[1] + (d == 1) && z0 + c < L.n[2] + (d == 2);
   if (!valid) return;
