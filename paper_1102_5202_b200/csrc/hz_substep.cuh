@@ -41,6 +41,7 @@ struct TileGeom {
   static constexpr int WX = NFX / 32, WY = NFY / 32, WZ = NFZ / 32;  // warp tasks per direction
   static_assert(NFX % 32 == 0 && NFY % 32 == 0 && NFZ % 32 == 0, "face lists must split into whole warps");
   static_assert(NC == NT, "phase 2 maps one cell to one thread");
+  static_assert(TY % 4 == 0, "the row swizzle permutes groups of four rows");
   static_assert(HX >= NG && (HX * sizeof(T)) % 16 == 0, "x halo: at least NG cells and 16-byte box rows starts");
   // staged boxes: primitives with halo 2, metric with halo 1; both with halo HX along x (same x origin)
   static constexpr int BX = TX + 2 * HX, BY = TY + 2 * NG, BZ = TZ + 2 * NG;
@@ -319,6 +320,12 @@ __device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __re
       }
 }
 
+// Row swizzle against shared-memory bank conflicts.  A warp item covers rows of TX cells; staged box rows
+// are BX = TX + 2 HX elements = 24 words apart, so rows b and b+1 read by one half-warp (fp64) or one
+// warp (fp32) overlap in 8 banks, while rows b and b+2 (48 words apart) do not.  Lanes that would take
+// rows (0,1,2,3) of a group of four take rows (0,2,1,3) instead: bits 0 and 1 of the row index swap.
+__device__ __forceinline__ int swz(int b) { return (b & ~3) | ((b & 1) << 1) | ((b >> 1) & 1); }
+
 // n / N for 0 <= n < NMAX and a compile-time N: shift or multiply-shift, never a division
 template <int N, int NMAX>
 __device__ __forceinline__ int cdiv(int n) {
@@ -351,7 +358,8 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
   const int r = d == 0 ? cdiv<G::TX + 1, G::NF>(f) : cdiv<G::TX, G::NF>(f);
   const int a = f - r * e0;
   const int c = d == 1 ? cdiv<G::TY + 1, G::NF>(r) : cdiv<G::TY, G::NF>(r);
-  const int b = r - c * e1;
+  const int b0 = r - c * e1;
+  const int b = b0 < (G::TY & ~3) ? swz(b0) : b0;   // the extra y face (b0 = TY) keeps its row
   // the face lies between cell (a,b,c) - e_d and cell (a,b,c)
   const bool valid = x0 + a < L.n[0] + (d == 0) && y0 + b < L.n[1] + (d == 1) && z0 + c < L.n[2] + (d == 2);
   if (!valid) return;
@@ -361,7 +369,7 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
   const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX) - sm;
   T Phi[NV];
   face_flux_rot<T>(sPc, sMc, sp, sm, d, par, Phi);
-  T* o = sF + off + f;
+  T* o = sF + off + (c * e1 + b) * e0 + a;
   o[0] = Phi[0];
   o[4 * G::NF] = Phi[4];
   o[8 * G::NF] = Phi[8];
@@ -380,7 +388,7 @@ __device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, 
                                             int cell, int x0, int y0, int z0) {
   using G = TileGeom<T>;
   const int a = cell % G::TX, r = cell / G::TX;
-  const int b = r % G::TY, c = r / G::TY;
+  const int b = swz(r % G::TY), c = r / G::TY;
   if (x0 + a >= L.n[0] || y0 + b >= L.n[1] || z0 + c >= L.n[2]) return;
   const T* sPc = sP + ((c + NG) * G::BY + (b + NG)) * G::BX + (a + G::HX);
   const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX);
@@ -445,7 +453,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
 
   // this thread's cell of phase 2 (one cell per thread), tile-local
   const int ca = threadIdx.x % G::TX, cr = threadIdx.x / G::TX;
-  const int cb = cr % G::TY, cc = cr / G::TY;
+  const int cb = swz(cr % G::TY), cc = cr / G::TY;
   const T* sPc = sP + ((cc + NG) * G::BY + (cb + NG)) * G::BX + (ca + G::HX);
   const T* sMc = sM + ((cc + 1) * G::MY + (cb + 1)) * G::BX + (ca + G::HX);
   int fail = 0, reset = 0, pfl = 0, it = 0;
