@@ -35,12 +35,12 @@ ALGO_WORDS_PATH = 52.0
 # Algorithmic flops per zone per substep (flops k_substep executes per zone by ncu,
 # 4120 in fp64 and 3190 in fp32, less the ~10 % that is duplicated tile-boundary face work; the plain
 # oracle counts 4564 add+mul, 648 div, 59 sqrt).  FMA = 2.
-ALGO_FLOPS = {"f64": 3700.0, "f32": 2900.0}
+ALGO_FLOPS = {"f64": 3700.0, "f32": 2900.0, "f32h": 2900.0}
 # ALU peak (B200_PROFILING.md unit counts): 148 SMs x lanes x 2 flop x max SM clock
-SMS, LANES = 148, {"f64": 64, "f32": 128}
+SMS, LANES = 148, {"f64": 64, "f32": 128, "f32h": 128}
 # ncu dram__bytes_read.sum + dram__bytes_write.sum of one k_substep launch at 128^3, per zone
 # (profiles/r01_substep.md); scaled to the launch's zones below
-TRAFFIC_BYTES_PER_ZONE = {"f64": 497.0, "f32": 268.0}
+TRAFFIC_BYTES_PER_ZONE = {"f64": 497.0, "f32": 268.0, "f32h": 268.0}
 
 
 def peaks():
@@ -308,7 +308,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=256, help="cells per axis of the Kerr-Schild sweep")
-    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32", "f32h"],
+                    help="f32h = fp32 storage and faces, fp64 flux difference / RK combine / con2prim (PAPER.md:126-128)")
     ap.add_argument("--ref-n", type=int, default=128, help="sub-grid the CPU oracle is timed on")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

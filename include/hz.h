@@ -43,7 +43,10 @@ extern "C" {
 
 typedef struct hz_ctx hz_ctx; /* opaque; created by hz_create, freed by hz_destroy */
 
-enum { HZ_F32 = 0, HZ_F64 = 1 };
+/* HZ_F32_F64: the paper's mixed mode: fields stored and face fluxes computed in
+ * fp32 (arrays at the boundary are float, as for HZ_F32); flux difference, Runge-Kutta combine and
+ * primitive recovery in fp64. */
+enum { HZ_F32 = 0, HZ_F64 = 1, HZ_F32_F64 = 2 };
 enum { HZ_BC_PERIODIC = 0, HZ_BC_OUTFLOW = 1 }; /* per axis */
 enum { HZ_OK = 0, HZ_EINVAL = -1, HZ_ENOMEM = -2, HZ_ECUDA = -3, HZ_ESTATE = -4 };
 

@@ -5,7 +5,7 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-HZ_F32, HZ_F64 = 0, 1
+HZ_F32, HZ_F64, HZ_F32_F64 = 0, 1, 2
 HZ_BC_PERIODIC, HZ_BC_OUTFLOW = 0, 1
 HZ_OK, HZ_EINVAL, HZ_ENOMEM, HZ_ECUDA, HZ_ESTATE = 0, -1, -2, -3, -4
 
@@ -131,8 +131,10 @@ class Horizon:
             self.dtype = HZ_F64
         elif dtype in ("f32", "float32", np.float32):
             self.dtype = HZ_F32
+        elif dtype in ("f32h", "f32_f64", "mixed"):
+            self.dtype = HZ_F32_F64      # fp32 storage and faces, fp64 flux difference / RK combine / con2prim
         else:
-            raise ValueError(f"dtype must be 'f64' or 'f32', got {dtype!r}")
+            raise ValueError(f"dtype must be 'f64', 'f32' or 'f32h', got {dtype!r}")
         self.np_dtype = np.float64 if self.dtype == HZ_F64 else np.float32
         self.grid = HzGrid(self.n[0], self.n[1], self.n[2], float(h[0]), float(h[1]), float(h[2]),
                            (C.c_int * 3)(*[int(b) for b in bc]))

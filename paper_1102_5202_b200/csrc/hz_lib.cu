@@ -132,7 +132,8 @@ Par<T> make_par(const hz_ctx* c) {
   p.p_atm = (T)h.p_atm;
   p.rho_thr = (T)(h.rho_atm * (1 + h.atm_tol));
   p.kappa = (T)h.kappa;
-  p.c2p_tol = (T)(h.c2p_tol > 0 ? h.c2p_tol : (sizeof(T) == 8 ? 1e-13 : 1e-6));
+  // dtype default of the Newton tolerance; in the mixed mode the fp64 recovery works on fp32 data
+  p.c2p_tol = (T)(h.c2p_tol > 0 ? h.c2p_tol : (c->dtype == HZ_F64 ? 1e-13 : (sizeof(T) == 8 ? 1e-10 : 1e-6)));
   p.c2p_maxit = h.c2p_maxit;
   p.cleaning = h.cleaning;
   for (int d = 0; d < 3; d++) p.ih[d] = (T)(1.0 / c->L.h[d]);
@@ -252,8 +253,14 @@ int substep_t(hz_ctx* c, double dt) {
   const unsigned grid = (unsigned)(ntiles < c->nsm ? ntiles : c->nsm);  // persistent: one block per SM
   {
     ProfScope ps(c, K_SUBSTEP);
-    k_substep<T><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, Uin, U0, Uout,
-                                                        c->P<T>(1 - c->pcur), st, (T)dt, c->counters(), ntx, nty, (int)ntiles);
+    if (sizeof(T) == 4 && c->dtype == HZ_F32_F64)  // fp32 storage and faces, fp64 flux difference / RK / con2prim
+      k_substep<float, double><<<grid, G::NT, G::SMEM, c->stream>>>(
+          c->tmP[c->pcur], c->tmM, L, make_par<float>(c), make_par<double>(c), (const float*)Uin, (const float*)U0,
+          (float*)Uout, (float*)c->P<T>(1 - c->pcur), st, dt, c->counters(), ntx, nty, (int)ntiles);
+    else
+      k_substep<T, T><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, par, Uin, U0, Uout,
+                                                            c->P<T>(1 - c->pcur), st, (T)dt, c->counters(), ntx, nty,
+                                                            (int)ntiles);
   }
   HZ_LAUNCHED(c);
   if (st == 0) { c->u0 = c->cur; c->cur = 1 - c->cur; }
@@ -296,7 +303,9 @@ int make_maps_t(hz_ctx* c) {
   for (int w = 0; w < 2; w++)
     if ((rc = make_tensor_map<T>(c->L, c->P<T>(w), NV, G::BY, G::BZ, &c->tmP[w]))) return rc;
   if ((rc = make_tensor_map<T>(c->L, c->met<T>(), NM, G::MY, G::MZ, &c->tmM))) return rc;
-  if (cudaFuncSetAttribute(k_substep<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM) != cudaSuccess) {
+  if (cudaFuncSetAttribute(k_substep<T, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(k_substep<float, double>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)TileGeom<float>::SMEM) != cudaSuccess) {
     cudaGetLastError();
     return HZ_ECUDA;
   }
@@ -373,7 +382,7 @@ int hz_default_params(hz_params* p) {
 }
 
 int hz_state_bytes(const hz_grid* grid, int dtype, size_t* bytes) {
-  if (!grid_ok(grid) || !bytes || (dtype != HZ_F32 && dtype != HZ_F64)) return HZ_EINVAL;
+  if (!grid_ok(grid) || !bytes || (dtype != HZ_F32 && dtype != HZ_F64 && dtype != HZ_F32_F64)) return HZ_EINVAL;
   *bytes = make_plan(make_layout(*grid, dtype), dtype).total;
   return HZ_OK;
 }
@@ -381,7 +390,7 @@ int hz_state_bytes(const hz_grid* grid, int dtype, size_t* bytes) {
 int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* device_buffer, hz_ctx** out) {
   if (!out) return HZ_EINVAL;
   *out = nullptr;
-  if (!grid_ok(grid) || (dtype != HZ_F32 && dtype != HZ_F64)) return HZ_EINVAL;
+  if (!grid_ok(grid) || (dtype != HZ_F32 && dtype != HZ_F64 && dtype != HZ_F32_F64)) return HZ_EINVAL;
   hz_params par;
   if (params) par = *params; else hz_default_params(&par);
   if (!(par.gamma_ad > 1) || par.c2p_maxit < 1 || !(par.rho_atm > 0) || !(par.p_atm > 0) || !(par.atm_tol >= 0))

@@ -429,11 +429,15 @@ __device__ __forceinline__ void issue_loads(const CUtensorMap* tmP, const CUtens
 // tmP / tmM: tensor maps of the current primitives and of the metric as 4D arrays (x, y, z, field).
 // Tiles are numbered x fastest; block b takes tiles b, b + gridDim.x, ...  While a block is in phase 2
 // of one tile, the TMA loads of its next tile are already in flight (the staged boxes are dead by then).
-template <typename T>
+// T2 is the arithmetic type of phase 2.  T2 = T: pure fp64 or pure fp32.  T = float with
+// T2 = double is the paper's mixed mode: storage, reconstruction and face fluxes in
+// fp32; flux difference, Runge-Kutta combine and the primitive recovery in fp64.
+template <typename T, typename T2>
 __global__ void __launch_bounds__(Tile<T>::NT, 1)
 k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmM, Layout L, Par<T> par,
-          const T* __restrict__ Uin, const T* __restrict__ U0, T* __restrict__ Uout, T* __restrict__ Pout, int stage,
-          T dt, unsigned long long* __restrict__ counters, int ntx, int nty, int ntiles) {
+          Par<T2> par2, const T* __restrict__ Uin, const T* __restrict__ U0, T* __restrict__ Uout,
+          T* __restrict__ Pout, int stage, T2 dt, unsigned long long* __restrict__ counters, int ntx, int nty,
+          int ntiles) {
   using G = TileGeom<T>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sP = reinterpret_cast<T*>(smem_raw + G::OFF_P);  // sP[field][z][y][x], halo 2 (HX in x)
@@ -499,84 +503,94 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       if (tile + (int)gridDim.x < ntiles) issue_loads<T>(&tmP, &tmM, L, sP, sM, bar, tile + gridDim.x, ntx, nty);
     }
 
-    // ---- phase 2: one cell per thread ----
+    // ---- phase 2: one cell per thread, arithmetic in T2 ----
     if (cell_ok) {
-      T R[NV];
+      T2 R[NV];
       R[0] = 0;
 #pragma unroll
-      for (int v = 1; v < NV; v++) R[v] = sR[(v - 1) * G::NC + threadIdx.x];
+      for (int v = 1; v < NV; v++) R[v] = (T2)sR[(v - 1) * G::NC + threadIdx.x];
       if (L.g[0]) {
-        const T ih = par.ih[0];
+        const T2 ih = par2.ih[0];
         const T* o = sF + (cc * G::TY + cb) * (G::TX + 1) + ca;
 #pragma unroll
-        for (int v = 0; v < NV; v++) R[v] -= (o[v * G::NF + 1] - o[v * G::NF]) * ih;
+        for (int v = 0; v < NV; v++) R[v] -= ((T2)o[v * G::NF + 1] - (T2)o[v * G::NF]) * ih;
       }
       if (L.g[1]) {
-        const T ih = par.ih[1];
+        const T2 ih = par2.ih[1];
         const T* o = sF + G::NFX + (cc * (G::TY + 1) + cb) * G::TX + ca;
 #pragma unroll
-        for (int v = 0; v < NV; v++) R[v] -= (o[v * G::NF + G::TX] - o[v * G::NF]) * ih;
+        for (int v = 0; v < NV; v++) R[v] -= ((T2)o[v * G::NF + G::TX] - (T2)o[v * G::NF]) * ih;
       }
       if (L.g[2]) {
-        const T ih = par.ih[2];
+        const T2 ih = par2.ih[2];
         const T* o = sF + G::NFX + G::NFY + (cc * G::TY + cb) * G::TX + ca;
 #pragma unroll
-        for (int v = 0; v < NV; v++) R[v] -= (o[v * G::NF + G::TX * G::TY] - o[v * G::NF]) * ih;
+        for (int v = 0; v < NV; v++) R[v] -= ((T2)o[v * G::NF + G::TX * G::TY] - (T2)o[v * G::NF]) * ih;
       }
-      if (!par.cleaning) R[8] = 0;
+      if (!par2.cleaning) R[8] = 0;
       // a7: Runge-Kutta stage combine
+      T2 un[NV];
 #pragma unroll
       for (int v = 0; v < NV; v++) {
-        T u1 = u[v] + dt * R[v];
-        if (stage == 1) u1 = T(0.75) * u0[v] + T(0.25) * u1;
-        if (stage == 2) u1 = T(1.0 / 3.0) * u0[v] + T(2.0 / 3.0) * u1;
-        u[v] = u1;
+        T2 u1 = (T2)u[v] + dt * R[v];
+        if (stage == 1) u1 = T2(0.75) * (T2)u0[v] + T2(0.25) * u1;
+        if (stage == 2) u1 = T2(1.0 / 3.0) * (T2)u0[v] + T2(2.0 / 3.0) * u1;
+        un[v] = u1;
       }
       // a8: primitive recovery and floors
-      T cf[6], gi[6];
-      const T det = cofactors(m + GXX, cf);
-      const T sq = sqrt_(det);
-      const T idet = rcp_(det);
+      T2 m2[NM], q2[NV];
+#pragma unroll
+      for (int v = 0; v < NM; v++) m2[v] = (T2)m[v];
+#pragma unroll
+      for (int v = 0; v < NV; v++) q2[v] = (T2)q[v];
+      T2 cf[6], gi[6];
+      const T2 det = cofactors(m2 + GXX, cf);
+      const T2 sq = sqrt_(det);
+      const T2 idet = rcp_(det);
 #pragma unroll
       for (int a6 = 0; a6 < 6; a6++) gi[a6] = cf[a6] * idet;
-      const T isq = rcp_(sq);
-      T w[NV];
+      const T2 isq = rcp_(sq);
+      T2 w[NV];
 #pragma unroll
-      for (int v = 0; v < NV; v++) w[v] = u[v] * isq;
-      if (!par.cleaning) w[8] = 0;
-      T Zg;
+      for (int v = 0; v < NV; v++) w[v] = un[v] * isq;
+      if (!par2.cleaning) w[8] = 0;
+      T2 Zg;
       {  // guess from the previous primitives of this cell
-        T utl[3];
-        lower(m + GXX, q + UX, utl);
-        const T W2 = 1 + dot3(q + UX, utl);
-        Zg = (q[RHO] + par.gg1 * q[PR]) * W2;
+        T2 utl[3];
+        lower(m2 + GXX, q2 + UX, utl);
+        const T2 W2 = 1 + dot3(q2 + UX, utl);
+        Zg = (q2[RHO] + par2.gg1 * q2[PR]) * W2;
       }
-      T qn[NV];
+      T2 qn[NV];
       int its = 0;
-      const int fl = con2prim(w, m, gi, par, Zg, qn, its);
+      const int fl = con2prim(w, m2, gi, par2, Zg, qn, its);
       it = its > it ? its : it;
       bool rs = fl != 0;
-      if (!rs && qn[RHO] < par.rho_thr) rs = true;
+      if (!rs && qn[RHO] < par2.rho_thr) rs = true;
       bool pf = false;
       if (rs) {
-        qn[RHO] = par.rho_atm; qn[PR] = par.p_atm;
+        qn[RHO] = par2.rho_atm; qn[PR] = par2.p_atm;
 #pragma unroll
         for (int a3 = 0; a3 < 3; a3++) { qn[UX + a3] = 0; qn[BX + a3] = w[5 + a3]; }
         qn[PSI] = w[8];
-      } else if (qn[PR] < par.p_atm) {
+      } else if (qn[PR] < par2.p_atm) {
         pf = true;
-        qn[PR] = par.p_atm;
+        qn[PR] = par2.p_atm;
       }
       if (rs || pf) {
-        T un[NV];
-        prim2con(qn, m, par, un);
+        T2 uf[NV];
+        prim2con(qn, m2, par2, uf);
 #pragma unroll
-        for (int v = 0; v < NV; v++) u[v] = sq * un[v];
+        for (int v = 0; v < NV; v++) un[v] = sq * uf[v];
       }
       fail += fl != 0; reset += rs; pfl += pf;
+      T qs[NV];
 #pragma unroll
-      for (int v = 0; v < NV; v++) Uout[v * L.fs + id] = u[v];
-      store_prims_with_images(L, Pout, ci, cj, ck, qn);
+      for (int v = 0; v < NV; v++) {
+        Uout[v * L.fs + id] = (T)un[v];
+        qs[v] = (T)qn[v];
+      }
+      store_prims_with_images(L, Pout, ci, cj, ck, qs);
     }
     __syncthreads();  // sF / sR may be overwritten by the next tile's phase 1
   }

@@ -55,6 +55,10 @@ def test_state_bytes_plan(L):
     n32 = C.c_size_t()
     assert L.hz_state_bytes(C.byref(grid(256, 256, 256)), B.HZ_F32, C.byref(n32)) == 0
     assert 0.45 * n.value < n32.value < 0.6 * n.value
+    # the mixed mode (fp32 storage, fp64 phase 2) stores exactly what fp32 stores
+    nmix = C.c_size_t()
+    assert L.hz_state_bytes(C.byref(grid(256, 256, 256)), B.HZ_F32_F64, C.byref(nmix)) == 0
+    assert nmix.value == n32.value
     # an inactive axis carries no ghosts: the tube is tiny
     assert L.hz_state_bytes(C.byref(grid(400, 1, 1)), B.HZ_F64, C.byref(n)) == 0
     assert n.value < 1 << 20

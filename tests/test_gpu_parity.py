@@ -78,6 +78,46 @@ def test_substep_parity_fp32(name):
     hz.close()
 
 
+@pytest.mark.parametrize("name", sorted(SMALL))
+def test_substep_parity_mixed_precision(name):
+    """The paper's mixed mode: fp32 storage and face fluxes, fp64 flux
+    difference, RK combine and con2prim.  Same bar as pure fp32 against the fp64 oracle."""
+    w = SMALL[name]()
+    o = oracle_for(w)
+    hz = horizon(w, "f32h")
+    o.substeps(w.dt, 1)
+    hz.substeps(w.dt, 1)
+    got = hz.get_primitives()
+    assert got.dtype == np.float32
+    ref = o.get_primitives()
+    flips = floor_flip_mask(got, ref, w.params["rho_atm"], w.params["atm_tol"])
+    assert flips.sum() <= 2e-4 * w.ncell, f"{flips.sum()} atmosphere-branch flips"
+    assert_parity(got, ref, TOL32_SUB, f"{name} mixed 1 substep", mask=flips)
+    hz.close()
+
+
+def test_mixed_precision_recovers_pressure_better_than_pure_fp32_on_the_star():
+    """Why the paper proposes fp64 islands: in fp32 the recovery of p from
+    tau + D loses digits where p << rho (the star's envelope and atmosphere, config 4).  After a full
+    RK3 step the pressure error of the mixed mode against the fp64 oracle must not exceed pure fp32's,
+    and the recovery must never fail in either."""
+    w = wl.tov_star(44)
+    o = oracle_for(w)
+    o.substeps(w.dt, 3)
+    ref = o.get_primitives()
+    err = {}
+    for dt in ("f32", "f32h"):
+        hz = horizon(w, dt)
+        hz.substeps(w.dt, 3)
+        got = hz.get_primitives().astype(np.float64)
+        d = hz.diagnostics()
+        assert d["c2p_fail"] == 0
+        err[dt] = rel_l1(got, ref)
+        hz.close()
+    assert err["f32h"]["p"] <= err["f32"]["p"] * 1.05, err
+    assert err["f32h"]["rho"] <= err["f32"]["rho"] * 1.05, err
+
+
 def test_full_run_config1_tube_fp64():
     """BASELINE config 1 exactly: 400 cells, CFL 0.4, 400 steps to t = 0.4."""
     w = wl.shock_tube(400)
