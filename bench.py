@@ -147,6 +147,21 @@ def run_reference(args):
     return 0
 
 
+def make_workload(wl, name, n):
+    """The five BASELINE.json configs at their stated sizes (kerr: n^3, the bench default 256^3)."""
+    if name == "kerr":
+        return wl.kerr_sweep(n), f"kerr_sweep_{n}^3 (BASELINE.json config 5: Kerr-Schild a=0.9, seeded torus, cleaning on)"
+    if name == "tube":
+        return wl.shock_tube(400), "shock_tube_400x1x1 (BASELINE.json config 1)"
+    if name == "alfven":
+        return wl.alfven_wave(64), "alfven_wave_64^3 (BASELINE.json config 2)"
+    if name == "blast":
+        return wl.blast(128), "blast_128^3 (BASELINE.json config 3)"
+    if name == "tov":
+        return wl.tov_star(192), "tov_star_192^3 (BASELINE.json config 4)"
+    raise ValueError(name)
+
+
 def max_over_ranks(ms, world, device):
     """Slowest rank's time: the only cross-rank operation of the replica path."""
     if world <= 1:
@@ -183,7 +198,7 @@ def run_gpu(args):
 
     n, dtype = args.n, args.dtype
     K, W = args.steps, max(args.warmup, 3)
-    w = wl.kerr_sweep(n)
+    w, wname = make_workload(wl, args.workload, n)
     stream = torch.cuda.current_stream()
     hz = Horizon.from_workload(w, dtype=dtype, stream=stream)
     es = 8 if dtype == "f64" else 4
@@ -281,8 +296,8 @@ def run_gpu(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": dtype, "data": "synthetic",
-        "config": {"workload": f"kerr_sweep_{n}^3 (BASELINE.json config 5: Kerr-Schild a=0.9, seeded torus, cleaning on)",
-                   "grid": [n, n, n], "substeps_per_step": SUBSTEPS_PER_STEP, "dt": w.dt,
+        "config": {"workload": wname,
+                   "grid": list(w.n), "substeps_per_step": SUBSTEPS_PER_STEP, "dt": w.dt,
                    "l2": "inputs larger than L2 (resident state %.1f GB)" % (hz.state_bytes / 1e9),
                    "parallelism": "replicas" if world > 1 else "single"},
         "clocks": clocks,
@@ -310,6 +325,8 @@ def main():
     ap.add_argument("--n", type=int, default=256, help="cells per axis of the Kerr-Schild sweep")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32", "f32h"],
                     help="f32h = fp32 storage and faces, fp64 flux difference / RK combine / con2prim (PAPER.md:126-128)")
+    ap.add_argument("--workload", default="kerr", choices=["kerr", "tube", "alfven", "blast", "tov"],
+                    help="which BASELINE.json config to time (default: config 5, the metric's workload)")
     ap.add_argument("--ref-n", type=int, default=128, help="sub-grid the CPU oracle is timed on")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
