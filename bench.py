@@ -200,13 +200,27 @@ def run_gpu(args):
     K, W = args.steps, max(args.warmup, 3)
     w, wname = make_workload(wl, args.workload, n)
     stream = torch.cuda.current_stream()
-    hz = Horizon.from_workload(w, dtype=dtype, stream=stream)
     es = 8 if dtype == "f64" else 4
-    ncell = w.ncell
+    shard = args.shard and world > 1
+    if shard:
+        # strong scaling: the ONE global box cut into `world` slabs along z, ghost planes exchanged over
+        # NCCL after every substep (paper_1102_5202_b200/slab.py)
+        from paper_1102_5202_b200 import DistSlabHorizon
+        from paper_1102_5202_b200.binding import HZ_HALO_PRIM
+        dsh = DistSlabHorizon(w, dtype=dtype)
+        hz = dsh.slab.hz
+        step = lambda: dsh.step(w.dt, 1)
+        ncell = dsh.slab.ncell                      # this rank's zones
+        total_cells = w.ncell                       # whole job
+    else:
+        hz = Horizon.from_workload(w, dtype=dtype, stream=stream)
+        step = lambda: hz.step(w.dt, 1)
+        ncell = w.ncell
+        total_cells = world * w.ncell               # replicas: every rank a full box
 
     # ---- device-resident timing: inputs in HBM, K x hz_step(dt, 1) --------------------------------
     for _ in range(W):
-        hz.step(w.dt, 1)
+        step()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -218,7 +232,7 @@ def run_gpu(args):
     t0 = time.time()
     e0.record(stream)
     for _ in range(K):
-        hz.step(w.dt, 1)
+        step()
     e1.record(stream)
     barrier()
     t1 = time.time()
@@ -228,7 +242,7 @@ def run_gpu(args):
     launches = hz.launch_count() - launches0
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     ms = max_over_ranks(ms, world, "cuda")
-    value = world * ncell * SUBSTEPS_PER_STEP * K / (ms * 1e-3)
+    value = total_cells * SUBSTEPS_PER_STEP * K / (ms * 1e-3)
     d = hz.diagnostics()
     finite = all(np.isfinite(v) for v in d.values())
 
@@ -238,21 +252,24 @@ def run_gpu(args):
     h_in = torch.from_numpy(hz.get_primitives()).to(td).pin_memory()
     h_out = torch.empty_like(h_in).pin_memory()
     Ke = max(1, min(K, args.e2e_steps))
-    for _ in range(2):
+    def e2e_step():
         hz.set_primitives(h_in)
-        hz.step(w.dt, 1)
+        if shard:
+            dsh.tr.exchange(dsh.slab, HZ_HALO_PRIM)
+        step()
         hz.get_primitives(out=h_out)
+
+    for _ in range(2):
+        e2e_step()
     barrier()
     e0.record(stream)
     for _ in range(Ke):
-        hz.set_primitives(h_in)
-        hz.step(w.dt, 1)
-        hz.get_primitives(out=h_out)
+        e2e_step()
     e1.record(stream)
     barrier()
     ms_e = e0.elapsed_time(e1)
     ms_e = max_over_ranks(ms_e, world, "cuda")
-    e2e_value = world * ncell * SUBSTEPS_PER_STEP * Ke / (ms_e * 1e-3)
+    e2e_value = total_cells * SUBSTEPS_PER_STEP * Ke / (ms_e * 1e-3)
     assert bool(torch.isfinite(h_out).all()), "non-finite primitives after the end-to-end steps"
 
     if rank != 0:
@@ -294,12 +311,12 @@ def run_gpu(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
         "dtype": dtype, "data": "synthetic",
         "config": {"workload": wname,
                    "grid": list(w.n), "substeps_per_step": SUBSTEPS_PER_STEP, "dt": w.dt,
                    "l2": "inputs larger than L2 (resident state %.1f GB)" % (hz.state_bytes / 1e9),
-                   "parallelism": "replicas" if world > 1 else "single"},
+                   "parallelism": ("z-slabs, NCCL halo exchange per substep" if shard else "replicas") if world > 1 else "single"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h_in.numel() * es),
                 "d2h_bytes_per_step": int(h_out.numel() * es), "steps": Ke, "ms_per_step": ms_e / Ke},
@@ -330,6 +347,9 @@ def main():
     ap.add_argument("--ref-n", type=int, default=128, help="sub-grid the CPU oracle is timed on")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--shard", action="store_true",
+                    help="with --gpus N > 1: cut the one box into N z-slabs with a halo exchange per substep "
+                         "(strong scaling) instead of N independent replicas (weak scaling, the default)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

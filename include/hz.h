@@ -47,7 +47,12 @@ typedef struct hz_ctx hz_ctx; /* opaque; created by hz_create, freed by hz_destr
  * fp32 (arrays at the boundary are float, as for HZ_F32); flux difference, Runge-Kutta combine and
  * primitive recovery in fp64. */
 enum { HZ_F32 = 0, HZ_F64 = 1, HZ_F32_F64 = 2 };
-enum { HZ_BC_PERIODIC = 0, HZ_BC_OUTFLOW = 1 }; /* per axis */
+/* Per axis.  The three EXTERNAL codes are for the z axis only (slab decomposition across GPUs,
+ * PAPER.md:176-178): the ghost planes of an external side are not filled by the library's boundary
+ * rule but supplied by the caller through hz_halo_unpack.  HZ_BC_EXTERNAL: both sides external;
+ * HZ_BC_EXTERNAL_OUTFLOW: low side external, high side outflow; HZ_BC_OUTFLOW_EXTERNAL: the reverse. */
+enum { HZ_BC_PERIODIC = 0, HZ_BC_OUTFLOW = 1, HZ_BC_EXTERNAL = 2, HZ_BC_EXTERNAL_OUTFLOW = 3,
+       HZ_BC_OUTFLOW_EXTERNAL = 4 };
 enum { HZ_OK = 0, HZ_EINVAL = -1, HZ_ENOMEM = -2, HZ_ECUDA = -3, HZ_ESTATE = -4 };
 
 /* Uniform Cartesian mesh.  An axis with one cell is inactive: no ghost zones, no
@@ -126,6 +131,22 @@ int hz_get_conserved(hz_ctx* ctx, void* cons9);
 
 /* Global reductions over the current state.  Synchronises the stream. */
 int hz_diagnostics(hz_ctx* ctx, hz_diag* out);
+
+/* Ghost-zone exchange of a slab decomposition along z (pack kernel, transfer, unpack
+ * kernel, every substep; here the transfer is device-to-device and the caller's: NCCL send/recv over
+ * NVLink between processes, or a plain copy between contexts of one process).  `which` selects the
+ * primitives (9 fields) or the metric (10 fields); `side` 0 = low z, 1 = high z.
+ * hz_halo_pack copies the NG = 2 interior planes next to that side -- whole padded planes, so the x and y
+ * ghost columns travel too -- into `device_buf` (hz_halo_bytes bytes, DEVICE memory, context dtype);
+ * hz_halo_unpack writes such a buffer into the ghost planes of that side.  A slab's low-side buffer
+ * goes to the high-side ghosts of the slab below it and vice versa.  Both are asynchronous on the context
+ * stream.  Call order per substep: hz_substeps(dt, 1) on every slab, pack, transfer, unpack; and once after
+ * hz_set_metric (metric) and after hz_set_primitives (primitives).  HZ_EINVAL if z is inactive or the
+ * buffer is not device memory; HZ_ESTATE before the fields are set. */
+enum { HZ_HALO_PRIM = 0, HZ_HALO_METRIC = 1 };
+int hz_halo_bytes(const hz_ctx* ctx, int which, size_t* bytes);
+int hz_halo_pack(hz_ctx* ctx, int which, int side, void* device_buf);
+int hz_halo_unpack(hz_ctx* ctx, int which, int side, const void* device_buf);
 
 /* Number of kernels this context has launched since hz_create (bench.py's gpu_launches). */
 long long hz_launch_count(const hz_ctx* ctx);

@@ -6,3 +6,4 @@ loudly if the library or a CUDA device is missing.
 """
 from .binding import (HZ_BC_OUTFLOW, HZ_BC_PERIODIC, HZ_F32, HZ_F32_F64, HZ_F64, Horizon, HzDiag, HzError, HzGrid, HzParams,
                       lib, lib_path)  # noqa: F401
+from .slab import DistSlabHorizon, SlabGroup  # noqa: F401

@@ -6,13 +6,14 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 HZ_F32, HZ_F64, HZ_F32_F64 = 0, 1, 2
-HZ_BC_PERIODIC, HZ_BC_OUTFLOW = 0, 1
+HZ_BC_PERIODIC, HZ_BC_OUTFLOW, HZ_BC_EXTERNAL, HZ_BC_EXTERNAL_OUTFLOW, HZ_BC_OUTFLOW_EXTERNAL = 0, 1, 2, 3, 4
+HZ_HALO_PRIM, HZ_HALO_METRIC = 0, 1
 HZ_OK, HZ_EINVAL, HZ_ENOMEM, HZ_ECUDA, HZ_ESTATE = 0, -1, -2, -3, -4
 
 # every symbol include/hz.h declares (tests check the library exports each of them)
 SYMBOLS = ["hz_default_params", "hz_state_bytes", "hz_create", "hz_destroy", "hz_set_stream", "hz_set_metric",
            "hz_set_primitives", "hz_step", "hz_substeps", "hz_get_primitives", "hz_get_psi", "hz_get_conserved",
-           "hz_diagnostics", "hz_launch_count", "hz_profile", "hz_profile_read", "hz_kernel_name",
+           "hz_diagnostics", "hz_halo_bytes", "hz_halo_pack", "hz_halo_unpack", "hz_launch_count", "hz_profile", "hz_profile_read", "hz_kernel_name",
            "hz_strerror"]
 HZ_NKERNELS = 4
 
@@ -88,6 +89,9 @@ def lib():
         L.hz_get_psi.argtypes = [vp, vp]
         L.hz_get_conserved.argtypes = [vp, vp]
         L.hz_diagnostics.argtypes = [vp, C.POINTER(HzDiag)]
+        L.hz_halo_bytes.argtypes = [vp, ip, C.POINTER(C.c_size_t)]
+        L.hz_halo_pack.argtypes = [vp, ip, ip, vp]
+        L.hz_halo_unpack.argtypes = [vp, ip, ip, vp]
         L.hz_launch_count.argtypes = [vp]
         L.hz_launch_count.restype = C.c_longlong
         L.hz_profile.argtypes = [vp, ip]
@@ -226,6 +230,19 @@ class Horizon:
         d = HzDiag()
         _chk(lib().hz_diagnostics(self._h, C.byref(d)), "hz_diagnostics")
         return d.asdict()
+
+    def halo_bytes(self, which):
+        n = C.c_size_t(0)
+        _chk(lib().hz_halo_bytes(self._h, int(which), C.byref(n)), "hz_halo_bytes")
+        return n.value
+
+    def halo_pack(self, which, side, buf):
+        """NG interior z planes next to `side` (0 low, 1 high) -> device buffer `buf` (torch CUDA tensor)."""
+        _chk(lib().hz_halo_pack(self._h, int(which), int(side), _ptr(buf)), "hz_halo_pack")
+
+    def halo_unpack(self, which, side, buf):
+        """Device buffer `buf` -> ghost z planes of `side`."""
+        _chk(lib().hz_halo_unpack(self._h, int(which), int(side), _ptr(buf)), "hz_halo_unpack")
 
     def launch_count(self):
         return lib().hz_launch_count(self._h)

@@ -43,6 +43,7 @@ __global__ void k_fill_ghosts(Layout L, T* __restrict__ F, int nf) {
   for (int d = 0; d < 3; d++) {
     const int n = L.n[d];
     if (c[d] < 0 || c[d] >= n) {
+      if (bc_side(L.bc[d], c[d] < 0 ? 0 : 1) == 2) return;  // external side: filled by hz_halo_unpack
       ghost = true;
       s[d] = L.bc[d] == 0 ? ((c[d] % n) + n) % n : (c[d] < 0 ? 0 : n - 1);
     } else {
@@ -52,6 +53,18 @@ __global__ void k_fill_ghosts(Layout L, T* __restrict__ F, int nf) {
   if (!ghost) return;
   const long long dst = L.idx(c[0], c[1], c[2]), src = L.idx(s[0], s[1], s[2]);
   for (int f = 0; f < nf; f++) F[f * L.fs + dst] = F[f * L.fs + src];
+}
+
+// ---- hz_halo_pack / hz_halo_unpack: NG whole padded z planes of nf fields <-> one contiguous buffer ----
+// k0: first storage plane; buffer layout [field][plane][y][x] with the padded extents of the context.
+template <typename T>
+__global__ void k_halo_copy(Layout L, T* __restrict__ F, int nf, int k0, T* __restrict__ buf, int unpack) {
+  const long long per = (long long)NG * L.sz, tot = per * nf;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < tot; e += (long long)gridDim.x * blockDim.x) {
+    const long long f = e / per, r = e - f * per;
+    T* cell = F + f * L.fs + (long long)k0 * L.sz + r;
+    if (unpack) *cell = buf[e]; else buf[e] = *cell;
+  }
 }
 
 // ---- hz_set_metric: interior-only planes -> padded SoA, with validation -------------------------

@@ -10,6 +10,15 @@
 
 namespace hz {
 
+// Boundary kind of one side of an axis (side 0 = low, 1 = high) from the per-axis code of hz_grid.bc:
+// 0 periodic, 1 outflow (zero gradient), 2 external (ghost layers are supplied through hz_halo_unpack;
+// only the z axis may be external).  Codes 3 / 4: external on the low / high side only, outflow on the other.
+__host__ __device__ inline int bc_side(int bc, int side) {
+  if (bc <= 2) return bc;
+  if (bc == 3) return side == 0 ? 2 : 1;
+  return side == 0 ? 1 : 2;
+}
+
 struct Layout {
   int n[3];        // interior cells per axis
   int g[3];        // ghost layers per side (NG on active axes, 0 on one-cell axes)

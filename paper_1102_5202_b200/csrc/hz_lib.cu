@@ -27,7 +27,8 @@ bool grid_ok(const hz_grid* G) {
   for (int d = 0; d < 3; d++) {
     if (n3[d] < 1) return false;
     if (n3[d] > 1 && n3[d] < NG) return false;
-    if (G->bc[d] != HZ_BC_PERIODIC && G->bc[d] != HZ_BC_OUTFLOW) return false;
+    const bool ext = G->bc[d] >= HZ_BC_EXTERNAL && G->bc[d] <= HZ_BC_OUTFLOW_EXTERNAL;
+    if (G->bc[d] != HZ_BC_PERIODIC && G->bc[d] != HZ_BC_OUTFLOW && !(ext && d == 2 && n3[d] >= NG)) return false;
   }
   return true;
 }
@@ -366,6 +367,25 @@ int diag_t(hz_ctx* c, hz_diag* out) {
   return HZ_OK;
 }
 
+// ---- slab decomposition along z: ghost planes of an external side (hz_halo_*) ----
+int halo_check(const hz_ctx* c, int which, int side) {
+  if (!c || (which != HZ_HALO_PRIM && which != HZ_HALO_METRIC) || (side != 0 && side != 1)) return HZ_EINVAL;
+  if (c->L.g[2] == 0) return HZ_EINVAL;
+  if (which == HZ_HALO_PRIM ? !c->have_prim : !c->have_metric) return HZ_ESTATE;
+  return HZ_OK;
+}
+
+template <typename T>
+int halo_copy_t(hz_ctx* c, int which, int k0, void* buf, int unpack) {
+  const int nf = which == HZ_HALO_PRIM ? NV : NM;
+  T* F = which == HZ_HALO_PRIM ? c->P<T>(c->pcur) : c->met<T>();
+  const long long tot = (long long)nf * NG * c->L.sz;
+  const unsigned nb = (unsigned)((tot + 255) / 256 < 4736 ? (tot + 255) / 256 : 4736);
+  k_halo_copy<T><<<nb, 256, 0, c->stream>>>(c->L, F, nf, k0, (T*)buf, unpack);
+  HZ_LAUNCHED(c);
+  return HZ_OK;
+}
+
 }  // namespace
 
 #define HZ_DISPATCH(c, fn, ...) ((c)->dtype == HZ_F64 ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
@@ -505,6 +525,30 @@ int hz_diagnostics(hz_ctx* c, hz_diag* out) {
   if (!c || !out) return HZ_EINVAL;
   if (!c->have_prim) return HZ_ESTATE;
   return HZ_DISPATCH(c, diag_t, c, out);
+}
+
+// ---- slab decomposition along z: ghost planes of an external side ----
+int hz_halo_bytes(const hz_ctx* c, int which, size_t* bytes) {
+  if (!c || !bytes || (which != HZ_HALO_PRIM && which != HZ_HALO_METRIC) || c->L.g[2] == 0) return HZ_EINVAL;
+  *bytes = (size_t)(which == HZ_HALO_PRIM ? NV : NM) * NG * (size_t)c->L.sz * elem_size(c->dtype);
+  return HZ_OK;
+}
+
+int hz_halo_pack(hz_ctx* c, int which, int side, void* device_buf) {
+  int rc = halo_check(c, which, side);
+  if (rc) return rc;
+  if (!device_buf || !is_device_ptr(device_buf)) return HZ_EINVAL;
+  // the NG interior planes next to that side: they become the neighbour's ghost planes
+  const int k0 = side == 0 ? c->L.g[2] : c->L.g[2] + c->L.n[2] - NG;
+  return HZ_DISPATCH(c, halo_copy_t, c, which, k0, device_buf, 0);
+}
+
+int hz_halo_unpack(hz_ctx* c, int which, int side, const void* device_buf) {
+  int rc = halo_check(c, which, side);
+  if (rc) return rc;
+  if (!device_buf || !is_device_ptr(device_buf)) return HZ_EINVAL;
+  const int k0 = side == 0 ? 0 : c->L.g[2] + c->L.n[2];
+  return HZ_DISPATCH(c, halo_copy_t, c, which, k0, const_cast<void*>(device_buf), 1);
 }
 
 long long hz_launch_count(const hz_ctx* c) { return c ? c->launches : 0; }

@@ -298,9 +298,9 @@ __device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __re
       if (L.bc[d] == 0) {  // periodic wrap
         if (c < NG) dst[d][cnt[d]++] = c + n;
         if (c >= n - NG) dst[d][cnt[d]++] = c - n;
-      } else {             // zero gradient: the edge cell fills its ghost layers
-        if (c == 0) { dst[d][1] = -1; dst[d][2] = -2; cnt[d] = 3; }
-        else if (c == n - 1) { dst[d][1] = n; dst[d][2] = n + 1; cnt[d] = 3; }
+      } else {             // zero gradient: the edge cell fills its ghost layers; external sides are left alone
+        if (c == 0 && bc_side(L.bc[d], 0) == 1) { dst[d][1] = -1; dst[d][2] = -2; cnt[d] = 3; }
+        else if (c == n - 1 && bc_side(L.bc[d], 1) == 1) { dst[d][1] = n; dst[d][2] = n + 1; cnt[d] = 3; }
       }
     }
     plain = plain && cnt[d] == 1;

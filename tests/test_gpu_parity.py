@@ -324,3 +324,60 @@ def test_errors_and_call_order():
     with pytest.raises(ValueError):
         hz.set_primitives(p[:, :4])
     hz.close()
+
+
+@pytest.mark.parametrize("make,parts,dtype", [
+    (lambda: wl.alfven_wave(n=(19, 12, 20)), 2, "f64"),     # periodic in z: the wrap-around is a neighbour
+    (lambda: wl.alfven_wave(n=(19, 12, 21)), 3, "f64"),     # uneven slabs
+    (lambda: wl.kerr_sweep(24), 3, "f64"),                  # outflow ends, curved metric (metric halos matter)
+    (lambda: wl.kerr_sweep(24), 2, "f32"),
+    (lambda: wl.blast(20), 4, "f32h"),
+])
+def test_slab_decomposition_reproduces_the_single_domain_bitwise(make, parts, dtype):
+    """Row f3: the domain cut into slabs along z, ghost planes exchanged through
+    hz_halo_pack / hz_halo_unpack after every substep, must give the single-context result bit for bit
+    (same per-face and per-cell arithmetic; only where the ghost values come from differs)."""
+    from paper_1102_5202_b200 import SlabGroup
+    w = make()
+    one = horizon(w, dtype)
+    grp = SlabGroup(w, parts, dtype)
+    one.substeps(w.dt, 4)
+    grp.substeps(w.dt, 4)
+    a, b = one.get_primitives(), grp.get_primitives()
+    assert a.shape == b.shape
+    assert np.array_equal(a, b), f"max |diff| = {np.abs(a - b).max()}"
+    da, db = one.diagnostics(), grp.diagnostics()
+    for k in ("c2p_fail", "atm_reset", "p_floor"):
+        assert da[k] == db[k]
+    for k in ("divB_max", "max_speed_over_dx"):
+        assert da[k] == db[k]
+    for k in ("sumD", "sumTau", "sumBx", "divB_L1"):
+        assert abs(da[k] - db[k]) <= 1e-12 * max(abs(da[k]), 1e-300) + 1e-30, k
+    one.close()
+    grp.close()
+
+
+def test_halo_calls_report_errors():
+    from paper_1102_5202_b200 import binding as B
+    import torch
+    w = wl.shock_tube(64, axis=0)            # z inactive
+    hz = horizon(w, "f64")
+    with pytest.raises(B.HzError) as e:
+        hz.halo_bytes(B.HZ_HALO_PRIM)
+    assert e.value.code == B.HZ_EINVAL
+    hz.close()
+    w = wl.alfven_wave(n=(8, 8, 8))
+    hz = horizon(w, "f64")
+    nbytes = hz.halo_bytes(B.HZ_HALO_PRIM)
+    assert nbytes == 9 * 2 * hz.halo_bytes(B.HZ_HALO_METRIC) // (10 * 2)
+    host = np.empty(nbytes, dtype=np.uint8)
+    with pytest.raises(B.HzError) as e:
+        hz.halo_pack(B.HZ_HALO_PRIM, 0, host)          # host memory is refused
+    assert e.value.code == B.HZ_EINVAL
+    buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.HzError) as e:
+        hz.halo_pack(B.HZ_HALO_PRIM, 2, buf)
+    assert e.value.code == B.HZ_EINVAL
+    hz.halo_pack(B.HZ_HALO_PRIM, 1, buf)
+    hz.halo_unpack(B.HZ_HALO_PRIM, 1, buf)
+    hz.close()
