@@ -504,8 +504,11 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     }
 
     // ---- phase 2: one cell per thread, arithmetic in T2 ----
+    // 2a: right-hand side from the fluxes and sources in shared memory; after the barrier below sF / sR are
+    // free, so a warp that finishes 2b early goes straight on to the next tile's work queue (the Newton
+    // iteration counts differ from cell to cell, and no barrier follows them).
+    T2 R[NV];
     if (cell_ok) {
-      T2 R[NV];
       R[0] = 0;
 #pragma unroll
       for (int v = 1; v < NV; v++) R[v] = (T2)sR[(v - 1) * G::NC + threadIdx.x];
@@ -528,6 +531,9 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
         for (int v = 0; v < NV; v++) R[v] -= ((T2)o[v * G::NF + G::TX * G::TY] - (T2)o[v * G::NF]) * ih;
       }
       if (!par2.cleaning) R[8] = 0;
+    }
+    __syncthreads();  // everybody has read sF / sR: the next tile's phase 1 may overwrite them
+    if (cell_ok) {  // 2b
       // a7: Runge-Kutta stage combine
       T2 un[NV];
 #pragma unroll
@@ -592,7 +598,6 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       }
       store_prims_with_images(L, Pout, ci, cj, ck, qs);
     }
-    __syncthreads();  // sF / sR may be overwritten by the next tile's phase 1
   }
   // warp-level reduction of the counters: [0] c2p_fail, [1] atm_reset, [2] p_floor, [3] max iterations
   const unsigned full = 0xffffffffu;
