@@ -168,13 +168,14 @@ def test_diagnostics_match_oracle():
     hz.close()
 
 
-def test_bench_configuration_sampled_block_256():
-    """BASELINE config 5 at the bench size (256^3, fp64, the launch configuration bench.py times):
+@pytest.mark.parametrize("dtype,tol", [("f64", TOL64_SUB * 10), ("f32", TOL32_SUB * 3), ("f32h", TOL32_SUB * 3)])
+def test_bench_configuration_sampled_block_256(dtype, tol):
+    """BASELINE config 5 at the bench size (256^3, the launch configuration bench.py times), all three modes:
     after one full RK3 step a cell depends only on cells within 3 x 3 zones of it (two for the MC
     stencil, one for the source differences, per substep), so the oracle run on a 44^3 sub-block of the
     same inputs fixes the inner 20^3 cells one by one."""
     w = wl.kerr_sweep(256)
-    hz = horizon(w, "f64")
+    hz = horizon(w, dtype)
     hz.step(w.dt, 1)
     got = hz.get_primitives()
     assert np.isfinite(got).all()
@@ -188,7 +189,7 @@ def test_bench_configuration_sampled_block_256():
         lo = [0 if s.start == 0 else m for s in sl]          # a true domain boundary needs no margin
         inner = tuple(slice(a, 44 - m) for a in lo)
         g = got[(slice(None),) + sl][(slice(None),) + inner]
-        assert_parity(g, ref[(slice(None),) + inner], TOL64_SUB * 10, f"256^3 block at {(k0, j0, i0)}")
+        assert_parity(g, ref[(slice(None),) + inner], tol, f"256^3 {dtype} block at {(k0, j0, i0)}")
     hz.close()
 
 
