@@ -387,6 +387,7 @@ __device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, con
   }
   if (!(v2 < 1)) return 1;
   bool ok = false;
+  T dZ = Z;
   for (int it = 1; it <= par.c2p_maxit; it++) {
     iters = it;
     T Zn = Z - div_(f, df);
@@ -402,10 +403,16 @@ __device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, con
       if (++halv > 40) return 1;
       Zn = (Z + Zn) * T(0.5);
     }
-    T dZ = abs_(Zn - Z);
+    dZ = abs_(Zn - Z);
     Z = Zn; v2 = v2n; f = fn; df = dfn;
-    if (dZ <= par.c2p_tol * Z) { ok = true; break; }
+    // fp64: |dZ| <= tol Z (R11).  fp32: the round-off of f is eps * (Z + B^2), so where the field
+    // dominates (B^2 > Z) the step cannot fall below that; the test is made against Z + B^2 there.
+    const T scale = sizeof(T) == 4 ? Z + c.B2 : Z;
+    if (dZ <= par.c2p_tol * scale) { ok = true; break; }
   }
+  // fp32 only: an iteration that has stalled at the round-off floor (last step below 1e-4 of the scale) has
+  // found the root to working precision; resetting such a cell to atmosphere would be the larger error.
+  if (!ok && sizeof(T) == 4 && dZ <= T(1e-4) * (Z + c.B2)) ok = true;
   if (!ok) return 1;
   const T omv = 1 - v2;
   const T sq = sqrt_(omv);
