@@ -154,6 +154,30 @@ def test_full_run_parity_fp64(name, make, nsteps):
     hz.close()
 
 
+@pytest.mark.parametrize("name,make", [
+    ("blast128", lambda: wl.blast(128)),        # BASELINE config 3 exactly: 128^3, 67 steps = 201 substeps
+    ("kerr128", lambda: wl.kerr_sweep(128)),    # BASELINE config 5 at 128^3: 34 steps = 102 substeps
+])
+def test_full_run_parity_at_baseline_size_fp64(name, make):
+    """Full-length runs at BASELINE.json's own sizes against the oracle (about two minutes of oracle time on
+    16 host cores): every cell, rel. L1 <= 1e-7 per field, identical floor and failure counts."""
+    w = make()
+    o = oracle_for(w)
+    hz = horizon(w, "f64")
+    hz.step(w.dt, w.nsteps)
+    o.step(w.dt, w.nsteps)
+    got = hz.get_primitives()
+    assert np.isfinite(got).all()
+    r = assert_parity(got, o.get_primitives(), TOL64_RUN, f"{name} {w.nsteps} steps")
+    do, dg = o.diagnostics(), hz.diagnostics()
+    for k in ("c2p_fail", "atm_reset", "p_floor"):
+        assert do[k] == dg[k], (k, do[k], dg[k])
+    for k in ("sumD", "sumTau"):
+        assert abs(do[k] - dg[k]) <= 1e-9 * abs(do[k]), (k, do[k], dg[k])
+    print(name, "max rel L1", max(r.values()))
+    hz.close()
+
+
 def test_diagnostics_match_oracle():
     w = wl.kerr_sweep(33)
     o = oracle_for(w)
