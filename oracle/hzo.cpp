@@ -304,7 +304,9 @@ C2PIn c2p_input(const Cons& w, const Met& m, const Geo& geo) {
   return c;
 }
 // Newton iteration on Z.  Returns 0 on convergence (prim filled, floors NOT applied), 1 on failure.
+int con2prim_2d(const Cons& w, const Met& m, const hzo_params& par, real Zguess, Prim* out, int* iters);
 int con2prim(const Cons& w, const Met& m, const hzo_params& par, real Zguess, Prim* out, int* iters) {
+  if (par.c2p_scheme == 1) return con2prim_2d(w, m, par, Zguess, out, iters);
   Geo geo = geometry(m);
   C2PIn c = c2p_input(w, m, geo);
   real Gam = par.gamma_ad;
@@ -347,6 +349,71 @@ int con2prim(const Cons& w, const Met& m, const hzo_params& par, real Zguess, Pr
   Prim q;
   q.rho = c.D / W;
   q.p = (Gam - 1) / Gam * (Z * omv - c.D * r_sqrt(omv));
+  for (int i = 0; i < 3; i++) {
+    real Su = 0;
+    for (int j = 0; j < 3; j++) Su += geo.gi[i][j] * w.S[j];
+    real vi = Su / (Z + c.B2) + c.SB * w.B[i] / (Z * (Z + c.B2));
+    q.ut[i] = W * vi;
+    q.B[i] = w.B[i];
+  }
+  q.psi = w.psi;
+  if (!r_finite(q.rho) || !r_finite(q.p) || !r_finite(W)) return 1;
+  *out = q;
+  return 0;
+}
+
+// O8b.  The same root by a Newton iteration on TWO unknowns (Z, v^2) -- reading R10b of PAPER.md:128
+// ("1D_P or 2D_W methods from Noble et al."): the unknown v^2 is not eliminated but iterated with Z,
+//   g1(Z, v2) = v2 - V(Z) = 0,   V(Z) = [S^2 Z^2 + SB^2 (B^2 + 2Z)] / [Z^2 (Z + B^2)^2]
+//   g2(Z, v2) = Z - p(Z, v2) + B^2 (1 + v2)/2 - SB^2/(2 Z^2) - E = 0,   p = (G-1)/G [Z (1 - v2) - D sqrt(1 - v2)]
+// with the 2x2 Jacobian  [[-V'(Z), 1], [dg2/dZ, dg2/dv2]].  Same root as O8 (it is unique), other iterates.
+int con2prim_2d(const Cons& w, const Met& m, const hzo_params& par, real Zguess, Prim* out, int* iters) {
+  Geo geo = geometry(m);
+  C2PIn c = c2p_input(w, m, geo);
+  real Gam = par.gamma_ad, gg = (Gam - 1) / Gam;
+  *iters = 0;
+  if (!(w.D > 0) || !r_finite(w.D) || !r_finite(c.S2) || !r_finite(c.E) || !r_finite(c.B2)) return 1;
+  real Z = Zguess;
+  if (!(Z > 0) || !r_finite(Z)) Z = c.E + c.D;
+  if (!(Z > 0)) Z = c.D;
+  real V, f1d, df1d;
+  for (int k = 0; k < 200; k++) {   // start inside v^2 < 1
+    c2p_eval(Z, c, Gam, &V, &f1d, &df1d);
+    if (V < 1 && r_finite(f1d)) break;
+    Z = 2 * Z;
+  }
+  if (!(V < 1)) return 1;
+  real v2 = V;
+  bool ok = false;
+  for (int it = 1; it <= par.c2p_maxit; it++) {
+    *iters = it;
+    real ZB = Z + c.B2, SB2 = c.SB * c.SB;
+    real Vz = (c.S2 * Z * Z + SB2 * (c.B2 + 2 * Z)) / (Z * Z * ZB * ZB);
+    real dV = -2 * (c.S2 * Z * Z * Z + SB2 * (3 * Z * Z + 3 * Z * c.B2 + c.B2 * c.B2)) / (Z * Z * Z * ZB * ZB * ZB);
+    real omv = 1 - v2, sq = r_sqrt(omv);
+    real p = gg * (Z * omv - c.D * sq);
+    real g1 = v2 - Vz;
+    real g2 = Z - p + c.B2 * (1 + v2) / 2 - SB2 / (2 * Z * Z) - c.E;
+    real a = 1 - gg * omv + SB2 / (Z * Z * Z);                 // dg2/dZ
+    real b = -gg * (-Z + c.D / (2 * sq)) + c.B2 / 2;           // dg2/dv2
+    real dZ = (-g2 + b * g1) / (a + b * dV);
+    real dv = -g1 + dV * dZ;
+    real Zn = Z + dZ, vn = v2 + dv;
+    int halv = 0;
+    while (!(r_finite(Zn) && Zn > 0 && r_finite(vn) && vn < 1 && vn >= 0)) {   // stay in the physical region
+      if (++halv > 40) return 1;
+      dZ = dZ / 2; dv = dv / 2;
+      Zn = Z + dZ; vn = v2 + dv;
+    }
+    Z = Zn; v2 = vn;
+    if (r_abs(dZ) <= par.c2p_tol * Z && r_abs(dv) <= par.c2p_tol) { ok = true; break; }
+  }
+  if (!ok) return 1;
+  real omv = 1 - v2;
+  real W = 1 / r_sqrt(omv);
+  Prim q;
+  q.rho = c.D / W;
+  q.p = gg * (Z * omv - c.D * r_sqrt(omv));
   for (int i = 0; i < 3; i++) {
     real Su = 0;
     for (int j = 0; j < 3; j++) Su += geo.gi[i][j] * w.S[j];
@@ -674,7 +741,7 @@ int hzo_default_params(hzo_params* p) {
   p->gamma_ad = 4.0 / 3.0;
   p->rho_atm = 1e-12; p->p_atm = 1e-14; p->atm_tol = 1e-3;
   p->cleaning = 1; p->kappa = 1.0;
-  p->c2p_maxit = 30; p->c2p_tol = 1e-13;
+  p->c2p_maxit = 30; p->c2p_tol = 1e-13; p->c2p_scheme = 0;
   return HZO_OK;
 }
 

@@ -43,6 +43,7 @@ typedef struct {
   double kappa;            /* cleaning damping rate                                  */
   int    c2p_maxit;        /* Newton iteration cap                                   */
   double c2p_tol;          /* |dZ| <= tol*Z                                          */
+  int    c2p_scheme;       /* 0: Newton on Z (O8); 1: Newton on (Z, v^2) (O8b)       */
 } hzo_params;
 
 typedef struct {

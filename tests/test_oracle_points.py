@@ -298,3 +298,47 @@ def test_con2prim_guess_independence_and_failure():
     assert ob.con2prim_point(w, flat, par)[0] == 1
     w = np.array([1.0, np.nan, 0, 0, 1.0, 0, 0, 0, 0])
     assert ob.con2prim_point(w, flat, par)[0] == 1
+
+
+# ---- O8b: the two-unknown scheme (reading R10b) ----------------------------------------
+def test_two_unknown_scheme_roundtrip_and_agreement_with_the_one_unknown_scheme():
+    """The physical root is unique, so Newton on (Z, v^2) must return the primitives Newton on Z returns
+    (two different iterations, one answer), and it must pass the P1 round trip on its own: 1e-12 for
+    E/p <= 1e3.  Both start from the built-in guess."""
+    P, M = states(43, 4000)
+    par1 = OracleParams.default(gamma_ad=GAM)
+    par2 = OracleParams.default(gamma_ad=GAM, c2p_scheme=1)
+    nchk, worst_rt, worst_ag = 0, 0.0, 0.0
+    for q, m in zip(P, M):
+        w = ob.prim2con_point(q, m, GAM)
+        g = gamma3(m)
+        if (w[4] + w[0]) / q[4] > 1e3 or np.linalg.cond(g) > 20:
+            continue
+        rc1, a, it1 = ob.con2prim_point(w, m, par1)
+        rc2, b, it2 = ob.con2prim_point(w, m, par2)
+        assert rc1 == 0 and rc2 == 0 and it2 <= 30, (rc1, rc2, it2)
+        un = np.sqrt(1 + q[1:4] @ g @ q[1:4])
+        dist = lambda x, y: max(abs(x[0] - y[0]) / y[0], abs(x[4] - y[4]) / y[4],
+                                np.sqrt((x[1:4] - y[1:4]) @ g @ (x[1:4] - y[1:4])) / un)
+        worst_rt = max(worst_rt, dist(b, q))
+        worst_ag = max(worst_ag, dist(b, a))
+        assert np.array_equal(b[5:9], q[5:9])
+        nchk += 1
+    assert nchk > 2000
+    assert worst_rt <= 1e-12, worst_rt
+    assert worst_ag <= 1e-12, worst_ag
+
+
+def test_two_unknown_scheme_is_a_different_iteration():
+    """Guard against the second scheme silently calling the first: from a poor guess the two take
+    different numbers of steps on some states."""
+    P, M = states(44, 300)
+    par1 = OracleParams.default(gamma_ad=GAM)
+    par2 = OracleParams.default(gamma_ad=GAM, c2p_scheme=1)
+    differ = 0
+    for q, m in zip(P, M):
+        w = ob.prim2con_point(q, m, GAM)
+        it1 = ob.con2prim_point(w, m, par1)[2]
+        it2 = ob.con2prim_point(w, m, par2)[2]
+        differ += it1 != it2
+    assert differ > 30, differ
