@@ -398,13 +398,23 @@ int con2prim_2d(const Cons& w, const Met& m, const hzo_params& par, real Zguess,
     real b = -gg * (-Z + c.D / (2 * sq)) + c.B2 / 2;           // dg2/dv2
     real dZ = (-g2 + b * g1) / (a + b * dV);
     real dv = -g1 + dV * dZ;
-    real Zn = Z + dZ, vn = v2 + dv;
+    // Trial point.  Far from the root the linearised v2 can leave [0, 1) (V is steep at small Z): such a
+    // trial is put back on the curve v2 = V(Z); a trial that is still unphysical halves the step.
+    real Zn, vn;
     int halv = 0;
-    while (!(r_finite(Zn) && Zn > 0 && r_finite(vn) && vn < 1 && vn >= 0)) {   // stay in the physical region
+    for (;;) {
+      Zn = Z + dZ; vn = v2 + dv;
+      bool good = r_finite(Zn) && Zn > 0;
+      if (good && !(r_finite(vn) && vn >= 0 && vn < 1)) {
+        real ZBn = Zn + c.B2;
+        vn = (c.S2 * Zn * Zn + SB2 * (c.B2 + 2 * Zn)) / (Zn * Zn * ZBn * ZBn);
+      }
+      good = good && r_finite(vn) && vn >= 0 && vn < 1;
+      if (good) break;
       if (++halv > 40) return 1;
       dZ = dZ / 2; dv = dv / 2;
-      Zn = Z + dZ; vn = v2 + dv;
     }
+    dv = vn - v2;
     Z = Zn; v2 = vn;
     if (r_abs(dZ) <= par.c2p_tol * Z && r_abs(dv) <= par.c2p_tol) { ok = true; break; }
   }

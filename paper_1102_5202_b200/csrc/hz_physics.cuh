@@ -27,6 +27,7 @@ struct Par {
   T c2p_tol;
   T ih[3];     // 1/dx, 1/dy, 1/dz
   int c2p_maxit;
+  int c2p_scheme;  // 0: Newton on Z, 1: Newton on (Z, v^2)
   int cleaning;
 };
 
@@ -363,7 +364,7 @@ __device__ __forceinline__ void c2p_eval(T Z, const C2P<T>& c, const Par<T>& par
 
 // w: undensitised conserved; gi: inverse 3-metric (packed); Zg: guess.  Returns 0 on success.
 template <typename T>
-__device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters) {
+__device__ __forceinline__ int con2prim_1d(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters) {
   C2P<T> c;
   T Su[3], Bl[3];
   lower(gi, w + 1, Su);
@@ -429,6 +430,95 @@ __device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, con
   q[PSI] = w[8];
   if (!finite_(q[RHO]) || !finite_(q[PR]) || !finite_(W)) return 1;
   return 0;
+}
+
+// ---- O8b: the same root by Newton on the two unknowns (Z, v^2) ("2D_W"; R10b) ----
+//   g1 = v2 - V(Z),  g2 = Z - p(Z, v2) + B^2 (1 + v2)/2 - SB^2/(2 Z^2) - E,  Jacobian [[-V', 1], [a, b]]
+template <typename T>
+__device__ __forceinline__ int con2prim_2d(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters) {
+  C2P<T> c;
+  T Su[3], Bl[3];
+  lower(gi, w + 1, Su);
+  lower(m + GXX, w + 5, Bl);
+  c.D = w[0];
+  c.S2 = dot3(w + 1, Su);
+  c.B2 = dot3(w + 5, Bl);
+  c.SB = dot3(w + 1, w + 5);
+  c.E = w[4] + w[0];
+  iters = 0;
+  if (!(c.D > 0) || !finite_(c.D) || !finite_(c.S2) || !finite_(c.E) || !finite_(c.B2)) return 1;
+  T Z = Zg;
+  if (!(Z > 0) || !finite_(Z)) Z = c.E + c.D;
+  if (!(Z > 0)) Z = c.D;
+  T v2, f, df;
+  for (int k = 0; k < 200; k++) {  // start inside v^2 < 1
+    c2p_eval(Z, c, par, v2, f, df);
+    if (v2 < 1 && finite_(f)) break;
+    Z = 2 * Z;
+  }
+  if (!(v2 < 1)) return 1;
+  const T SB2 = c.SB * c.SB;
+  bool ok = false;
+  T dZ = Z, dv = 1;
+  for (int it = 1; it <= par.c2p_maxit; it++) {
+    iters = it;
+    const T ZB = Z + c.B2, Z2 = Z * Z;
+    const T iZ = rcp_(Z), iZB = rcp_(ZB);
+    const T iZ2 = iZ * iZ, iZB2 = iZB * iZB;
+    const T V = (c.S2 * Z2 + SB2 * (c.B2 + 2 * Z)) * iZ2 * iZB2;
+    const T dV = -2 * (c.S2 * Z2 * Z + SB2 * (3 * Z2 + 3 * Z * c.B2 + c.B2 * c.B2)) * (iZ2 * iZ) * (iZB2 * iZB);
+    const T omv = 1 - v2, sq = sqrt_(omv);
+    const T p = par.g1g * (Z * omv - c.D * sq);
+    const T g1 = v2 - V;
+    const T g2 = Z - p + c.B2 * (1 + v2) * T(0.5) - SB2 * T(0.5) * iZ2 - c.E;
+    const T a = 1 - par.g1g * omv + SB2 * iZ2 * iZ;
+    const T b = -par.g1g * (-Z + div_(c.D, 2 * sq)) + c.B2 * T(0.5);
+    dZ = div_(-g2 + b * g1, a + b * dV);
+    dv = -g1 + dV * dZ;
+    // trial point: a linearised v2 outside [0, 1) is put back on the curve v2 = V(Z); a trial that is still
+    // unphysical halves the step
+    T Zn, vn;
+    int halv = 0;
+    for (;;) {
+      Zn = Z + dZ; vn = v2 + dv;
+      bool good = finite_(Zn) && Zn > 0;
+      if (good && !(finite_(vn) && vn >= 0 && vn < 1)) {
+        const T ZBn = Zn + c.B2;
+        vn = div_(c.S2 * Zn * Zn + SB2 * (c.B2 + 2 * Zn), Zn * Zn * ZBn * ZBn);
+      }
+      good = good && finite_(vn) && vn >= 0 && vn < 1;
+      if (good) break;
+      if (++halv > 40) return 1;
+      dZ = dZ * T(0.5); dv = dv * T(0.5);
+    }
+    dv = vn - v2;
+    Z = Zn; v2 = vn;
+    const T scale = sizeof(T) == 4 ? Z + c.B2 : Z;   // fp32: see con2prim_1d
+    if (abs_(dZ) <= par.c2p_tol * scale && abs_(dv) <= par.c2p_tol) { ok = true; break; }
+  }
+  if (!ok && sizeof(T) == 4 && abs_(dZ) <= T(1e-4) * (Z + c.B2) && abs_(dv) <= T(1e-4)) ok = true;
+  if (!ok) return 1;
+  const T omv = 1 - v2;
+  const T sq = sqrt_(omv);
+  const T W = rcp_(sq);
+  q[RHO] = c.D * sq;
+  q[PR] = par.g1g * (Z * omv - c.D * sq);
+  const T iZB = rcp_(Z + c.B2);
+  const T sbz = div_(c.SB, Z) * iZB;
+#pragma unroll
+  for (int i = 0; i < 3; i++) {
+    q[UX + i] = W * (Su[i] * iZB + sbz * w[5 + i]);
+    q[BX + i] = w[5 + i];
+  }
+  q[PSI] = w[8];
+  if (!finite_(q[RHO]) || !finite_(q[PR]) || !finite_(W)) return 1;
+  return 0;
+}
+
+template <typename T>
+__device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters) {
+  if (par.c2p_scheme == 1) return con2prim_2d(w, m, gi, par, Zg, q, iters);   // uniform over the launch
+  return con2prim_1d(w, m, gi, par, Zg, q, iters);
 }
 
 }  // namespace hz

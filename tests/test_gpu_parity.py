@@ -453,3 +453,38 @@ def test_pure_fp32_recovery_does_not_fail_in_the_magnetised_blast():
         hz.close()
     diff = np.abs(res["f32"] - res["f64"])
     assert diff[1:4].max() <= 1e-4 and diff[0].max() <= 1e-6 and diff[4].max() <= 1e-4, diff.reshape(8, -1).max(axis=1)
+
+
+@pytest.mark.parametrize("name", ["tube_x", "alfven_3d", "blast", "tov", "kerr"])
+def test_two_unknown_recovery_scheme_parity_and_agreement(name):
+    """Row f4 (the second con2prim scheme): Newton on (Z, v^2).  GPU against the oracle running
+    the same scheme at the fp64 bar after a full RK3 step; and, the root being unique, against the GPU's
+    own one-unknown run far below that bar.  fp32 at its bar."""
+    w = SMALL[name]()
+    w2 = dataclasses.replace(w, params={**w.params, "c2p_scheme": 1})
+    o = oracle_for(w2)
+    o.substeps(w.dt, 3)
+    ref = o.get_primitives()
+    hz2 = horizon(w2, "f64")
+    hz2.substeps(w.dt, 3)
+    got2 = hz2.get_primitives()
+    assert_parity(got2, ref, TOL64_SUB, f"{name} two-unknown scheme")
+    d2 = hz2.diagnostics()
+    do = o.diagnostics()
+    for k in ("c2p_fail", "atm_reset", "p_floor"):
+        assert d2[k] == do[k], (k, d2[k], do[k])
+    hz1 = horizon(w, "f64")
+    hz1.substeps(w.dt, 3)
+    assert_parity(got2, hz1.get_primitives(), 1e-11, f"{name} two-unknown vs one-unknown")
+    hz1.close()
+    hz2.close()
+    hz32 = horizon(w2, "f32")
+    o1 = oracle_for(w2)
+    o1.substeps(w.dt, 1)
+    hz32.substeps(w.dt, 1)
+    got = hz32.get_primitives()
+    ref1 = o1.get_primitives()
+    flips = floor_flip_mask(got, ref1, w.params["rho_atm"], w.params["atm_tol"])
+    assert flips.sum() <= 2e-4 * w.ncell
+    assert_parity(got, ref1, TOL32_SUB, f"{name} two-unknown scheme fp32", mask=flips)
+    hz32.close()
