@@ -70,6 +70,10 @@ typedef struct {
                           /* (1e-13 for HZ_F64, 1e-6 for HZ_F32)                                */
   int    c2p_scheme;      /* 0: Newton on Z = rho h W^2; 1: Newton on the two unknowns (Z, v^2),  */
                           /* the paper's second recovery scheme.  Same root.       */
+  int    energy_var;      /* 0: the energy slot of U is sqrt(gamma) tau (north_star); 1: the paper's */
+                          /* own variable -sqrt(-g) T^t_t = sqrt(gamma)[alpha(tau+D) - beta^j S_j]   */
+                          /* (PAPER.md:54, 60), which has no source on a fixed metric; hz_get_conserved */
+                          /* and hz_diag.sumTau then carry that variable.                            */
 } hz_params;
 
 /* Global reductions, all accumulated in fp64. */
@@ -83,7 +87,7 @@ typedef struct {
 } hz_diag;
 
 /* Fill *p with the defaults: Gamma = 4/3, atmosphere 1e-12 / 1e-14, atm_tol 1e-3, cleaning on,
- * kappa = 1, 30 Newton iterations, c2p_tol = 0 (dtype default), c2p_scheme = 0.  HZ_EINVAL if p is NULL. */
+ * kappa = 1, 30 Newton iterations, c2p_tol = 0 (dtype default), c2p_scheme = 0, energy_var = 0.  HZ_EINVAL if p is NULL. */
 int hz_default_params(hz_params* p);
 
 /* Bytes of device memory one context of this grid and dtype needs (all resident fields: metric,

@@ -135,6 +135,22 @@ Cons prim2con(const Prim& q, const Met& m, real Gam) {
 
 // O2.  Coordinate flux in direction d: alpha*F^d for D, S_j, tau (eq. 2 in 3+1
 // variables) and the cleaning rows for B^k, psi (reading R14).  Not times sqrt(gamma).
+// Reading R1b: the paper's own energy variable.  PAPER.md:54, 60 evolves sqrt(-g) T^t_t; with the 3+1
+// variables  -sqrt(-g) T^t_t = sqrt(gamma) [ alpha (tau + D) - beta^j S_j ]  (checked in O1).  For a
+// time-independent metric its source sqrt(-g) T^kappa_lambda Gamma^lambda_{t kappa} vanishes, so it is
+// conserved exactly.  These two maps swap slot 4 of an undensitised (D, S_j, tau, ..) vector (or of a
+// flux vector, the map being linear) between tau and that variable, on a given metric.
+void tau_to_energy(double* u9, const Met& m) {
+  real e = m.al * (real(u9[4]) + real(u9[0]));
+  for (int j = 0; j < 3; j++) e = e - m.be[j] * real(u9[1 + j]);
+  u9[4] = r_val(e);
+}
+void energy_to_tau(double* u9, const Met& m) {
+  real t = real(u9[4]);
+  for (int j = 0; j < 3; j++) t = t + m.be[j] * real(u9[1 + j]);
+  u9[4] = r_val(t / m.al - real(u9[0]));
+}
+
 void flux_of(int d, const Prim& q, const Met& m, const Geo& geo, real Gam, int cleaning, real* F) {
   Aux a = aux_of(q, m, Gam);
   Cons w = prim2con(q, m, Gam);
@@ -189,7 +205,7 @@ real mc_slope(real qm, real q0, real qp) {
 
 // O5.  HLLE flux through one face: needs only F(u_L), F(u_R) and the speeds.
 // Returns Phi = sqrt(gamma_f) * Fhat.
-void hlle(int d, const Prim& qL, const Prim& qR, const Met& mf, real Gam, int cleaning, real* Phi) {
+void hlle(int d, const Prim& qL, const Prim& qR, const Met& mf, real Gam, int cleaning, real* Phi, int energy_var = 0) {
   Geo geo = geometry(mf);
   real FL[NV], FR[NV], lmL, lpL, lmR, lpR;
   flux_of(d, qL, mf, geo, Gam, cleaning, FL);
@@ -199,6 +215,13 @@ void hlle(int d, const Prim& qL, const Prim& qR, const Met& mf, real Gam, int cl
   double uL[NV], uR[NV];
   store_cons(prim2con(qL, mf, Gam), uL);
   store_cons(prim2con(qR, mf, Gam), uR);
+  if (energy_var) {  // R1b: state and flux of the paper's energy variable, with the face metric
+    double fl[NV], fr[NV];
+    for (int c = 0; c < NV; c++) { fl[c] = r_val(FL[c]); fr[c] = r_val(FR[c]); }
+    // flux_of returns coordinate fluxes alpha F; the map is linear, so it applies to them as to the state
+    tau_to_energy(uL, mf); tau_to_energy(uR, mf); tau_to_energy(fl, mf); tau_to_energy(fr, mf);
+    FL[4] = fl[4]; FR[4] = fr[4];
+  }
   real lp = r_max(real(0), r_max(lpL, lpR));
   real lm = r_min(real(0), r_min(lmL, lmR));
   for (int c = 0; c < NV; c++) {
@@ -528,7 +551,7 @@ void face_flux(const hzo_ctx* c, int d, size_t id, real* Phi) {
   Rr.rho = r_max(Rr.rho, real(c->par.rho_atm)); Rr.p = r_max(Rr.p, real(c->par.p_atm));
   double mf[NM];
   for (int q = 0; q < NM; q++) mf[q] = 0.5 * (c->met[q][id] + c->met[q][id + s]);
-  hlle(d, L, Rr, load_met(mf), c->par.gamma_ad, c->par.cleaning, Phi);
+  hlle(d, L, Rr, load_met(mf), c->par.gamma_ad, c->par.cleaning, Phi, c->par.energy_var);
 }
 
 // O5 (flux difference) + O6 (sources): R = L(U) on interior cells.
@@ -594,6 +617,7 @@ void compute_rhs(hzo_ctx* c) {
         }
         real src4[4];
         fluid_source(q, m, dm, c->par.gamma_ad, src4);
+        if (c->par.energy_var) src4[3] = 0;   // R1b: no source for sqrt(-g) T^t_t on a fixed metric
         for (int a = 0; a < 4; a++) c->R[1 + a][id] += r_val(src4[a]);
         if (cleaning) {  // O6 cleaning sources (reading R14), not multiplied by alpha
           Geo geo = geometry(m);
@@ -626,6 +650,7 @@ void recover_primitives(hzo_ctx* c) {
         double w9[NV];
         for (int q = 0; q < NV; q++) w9[q] = c->U[q][id] / r_val(geo.sq);
         if (!c->par.cleaning) w9[8] = 0;
+        if (c->par.energy_var) energy_to_tau(w9, m);
         Cons w = load_cons(w9);
         Prim old = prim_at(c, id);
         Aux a = aux_of(old, m, c->par.gamma_ad);
@@ -652,6 +677,7 @@ void recover_primitives(hzo_ctx* c) {
         if (reset || pfl) {
           double u9[NV];
           store_cons(prim2con(q, m, c->par.gamma_ad), u9);
+          if (c->par.energy_var) tau_to_energy(u9, m);
           for (int v = 0; v < NV; v++) c->U[v][id] = r_val(geo.sq) * u9[v];
         }
       }
@@ -751,7 +777,7 @@ int hzo_default_params(hzo_params* p) {
   p->gamma_ad = 4.0 / 3.0;
   p->rho_atm = 1e-12; p->p_atm = 1e-14; p->atm_tol = 1e-3;
   p->cleaning = 1; p->kappa = 1.0;
-  p->c2p_maxit = 30; p->c2p_tol = 1e-13; p->c2p_scheme = 0;
+  p->c2p_maxit = 30; p->c2p_tol = 1e-13; p->c2p_scheme = 0; p->energy_var = 0;
   return HZO_OK;
 }
 
@@ -838,6 +864,7 @@ int hzo_set_primitives(hzo_ctx* c, const double* prim8) {
         double p9[NV], u9[NV];
         store_prim(q, p9);
         store_cons(prim2con(q, m, c->par.gamma_ad), u9);
+        if (c->par.energy_var) tau_to_energy(u9, m);
         real sq = geometry(m).sq;
         for (int v = 0; v < NV; v++) { c->P[v][id] = p9[v]; c->U[v][id] = r_val(sq) * u9[v]; }
       }

@@ -44,6 +44,8 @@ typedef struct {
   int    c2p_maxit;        /* Newton iteration cap                                   */
   double c2p_tol;          /* |dZ| <= tol*Z                                          */
   int    c2p_scheme;       /* 0: Newton on Z (O8); 1: Newton on (Z, v^2) (O8b)       */
+  int    energy_var;       /* 0: evolve sqrt(gamma) tau (R1); 1: the paper's          */
+                           /* -sqrt(-g) T^t_t (R1b): slot 4 of U, source-free        */
 } hzo_params;
 
 typedef struct {

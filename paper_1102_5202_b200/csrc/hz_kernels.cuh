@@ -122,6 +122,7 @@ __global__ void k_pack_prims(Layout L, Par<T> par, const T* __restrict__ prim8, 
   for (int a = 0; a < 3; a++) { q[UX + a] = W * a8[1 + a]; q[BX + a] = a8[5 + a]; }
   T w[NV];
   prim2con(q, m, par, w);
+  if (par.energy_var) w[4] = tau_to_energy(w, m);
   T sq = sqrt_det(m + GXX);
 #pragma unroll
   for (int v = 0; v < NV; v++) { P[v * L.fs + id] = q[v]; U[v * L.fs + id] = sq * w[v]; }

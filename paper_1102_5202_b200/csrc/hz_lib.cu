@@ -137,6 +137,7 @@ Par<T> make_par(const hz_ctx* c) {
   p.c2p_tol = (T)(h.c2p_tol > 0 ? h.c2p_tol : (c->dtype == HZ_F64 ? 1e-13 : (sizeof(T) == 8 ? 1e-10 : 1e-6)));
   p.c2p_maxit = h.c2p_maxit;
   p.c2p_scheme = h.c2p_scheme;
+  p.energy_var = h.energy_var;
   p.cleaning = h.cleaning;
   for (int d = 0; d < 3; d++) p.ih[d] = (T)(1.0 / c->L.h[d]);
   return p;
@@ -398,7 +399,7 @@ int hz_default_params(hz_params* p) {
   p->gamma_ad = 4.0 / 3.0;
   p->rho_atm = 1e-12; p->p_atm = 1e-14; p->atm_tol = 1e-3;
   p->cleaning = 1; p->kappa = 1.0;
-  p->c2p_maxit = 30; p->c2p_tol = 0.0; p->c2p_scheme = 0;
+  p->c2p_maxit = 30; p->c2p_tol = 0.0; p->c2p_scheme = 0; p->energy_var = 0;
   return HZ_OK;
 }
 
@@ -414,7 +415,7 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
   if (!grid_ok(grid) || (dtype != HZ_F32 && dtype != HZ_F64 && dtype != HZ_F32_F64)) return HZ_EINVAL;
   hz_params par;
   if (params) par = *params; else hz_default_params(&par);
-  if (!(par.gamma_ad > 1) || par.c2p_maxit < 1 || (par.c2p_scheme != 0 && par.c2p_scheme != 1) || !(par.rho_atm > 0) || !(par.p_atm > 0) || !(par.atm_tol >= 0))
+  if (!(par.gamma_ad > 1) || par.c2p_maxit < 1 || (par.c2p_scheme != 0 && par.c2p_scheme != 1) || (par.energy_var != 0 && par.energy_var != 1) || !(par.rho_atm > 0) || !(par.p_atm > 0) || !(par.atm_tol >= 0))
     return HZ_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return HZ_ECUDA; }

@@ -28,6 +28,7 @@ struct Par {
   T ih[3];     // 1/dx, 1/dy, 1/dz
   int c2p_maxit;
   int c2p_scheme;  // 0: Newton on Z, 1: Newton on (Z, v^2)
+  int energy_var;  // 0: slot 4 of U is tau; 1: the paper's -sqrt(-g) T^t_t / sqrt(gamma) (R1b)
   int cleaning;
 };
 
@@ -156,6 +157,19 @@ __device__ __forceinline__ double mc_slope<double>(double qm, double q0, double 
       : "=d"(s)
       : "d"(dm), "d"(dp));
   return s;
+}
+
+// ---- R1b: the paper's energy variable -------------------------------------------
+// -sqrt(-g) T^t_t = sqrt(gamma) [alpha (tau + D) - beta^j S_j]; source-free on a fixed metric.  The two maps
+// swap slot 4 of an undensitised (D, S_j, tau, ...) vector -- or, the map being linear, of a coordinate-flux
+// vector -- between tau and that variable on the metric m.
+template <typename T>
+__device__ __forceinline__ T tau_to_energy(const T* u, const T* m) {
+  return m[AL] * (u[4] + u[0]) - (m[BEX] * u[1] + m[BEY] * u[2] + m[BEZ] * u[3]);
+}
+template <typename T>
+__device__ __forceinline__ T energy_to_tau(const T* u, const T* m) {
+  return div_(u[4] + (m[BEX] * u[1] + m[BEY] * u[2] + m[BEZ] * u[3]), m[AL]) - u[0];
 }
 
 // ---- O1: everything one primitive state defines on a given metric -------------------------------

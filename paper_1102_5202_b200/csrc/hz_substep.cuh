@@ -158,6 +158,10 @@ __device__ __forceinline__ void state_flux0(const T* q, const T* m, const T* gi0
     for (int k = 1; k < 3; k++) F[5 + k] = vt * q[BX + k] - (al * (q[UX + k] * iW) - m[BEX + k]) * B0;
     F[8] = 0;
   }
+  if (par.energy_var) {  // R1b: state and coordinate flux of the paper's energy variable on the face metric
+    U[4] = tau_to_energy(U, m);
+    F[4] = tau_to_energy(F, m);
+  }
   // fast-speed bound a^2 = c_s^2 + v_A^2 - c_s^2 v_A^2 = (Gamma p + b^2)/(rho h + b^2)   (R7)
   T a2 = div_(par.Gam * q[PR] + b2, rhoh + b2);
   a2 = min_(max_(a2, T(0)), T(1));
@@ -407,6 +411,7 @@ __device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, 
 #pragma unroll
   for (int v = 0; v < NV; v++) R[v] = 0;
   add_sources_staged(L, sMc, m, q, par, gi, sq, R);
+  if (par.energy_var) R[4] = 0;  // R1b: no source on a fixed metric
 #pragma unroll
   for (int v = 1; v < NV; v++) sR[(v - 1) * G::NC + cell] = R[v];
 }
@@ -560,6 +565,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
 #pragma unroll
       for (int v = 0; v < NV; v++) w[v] = un[v] * isq;
       if (!par2.cleaning) w[8] = 0;
+      if (par2.energy_var) w[4] = energy_to_tau(w, m2);
       T2 Zg;
       {  // guess from the previous primitives of this cell
         T2 utl[3];
@@ -586,6 +592,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       if (rs || pf) {
         T2 uf[NV];
         prim2con(qn, m2, par2, uf);
+        if (par2.energy_var) uf[4] = tau_to_energy(uf, m2);
 #pragma unroll
         for (int v = 0; v < NV; v++) un[v] = sq * uf[v];
       }

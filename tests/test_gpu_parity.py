@@ -488,3 +488,42 @@ def test_two_unknown_recovery_scheme_parity_and_agreement(name):
     assert flips.sum() <= 2e-4 * w.ncell
     assert_parity(got, ref1, TOL32_SUB, f"{name} two-unknown scheme fp32", mask=flips)
     hz32.close()
+
+
+@pytest.mark.parametrize("name", ["tube_x", "alfven_3d", "tov", "kerr"])
+def test_papers_energy_variable_parity(name):
+    """Row f4 / reading R1b: evolve the paper's -sqrt(-g) T^t_t instead of sqrt(gamma) tau.
+    GPU against the oracle running the same option: primitives and the conserved set (slot 4 carries the
+    paper's variable) at the fp64 bar after a full RK3 step."""
+    w = SMALL[name]()
+    w1 = dataclasses.replace(w, params={**w.params, "energy_var": 1})
+    o = oracle_for(w1)
+    hz = horizon(w1, "f64")
+    o.substeps(w.dt, 3)
+    hz.substeps(w.dt, 3)
+    assert_parity(hz.get_primitives(), o.get_primitives(), TOL64_SUB, f"{name} energy variable")
+    Uo, Ug = o.get_conserved(), hz.get_conserved()
+    den = np.abs(Uo[4]).sum()
+    assert np.abs(Ug[4] - Uo[4]).sum() <= TOL64_SUB * den
+    do, dg = o.diagnostics(), hz.diagnostics()
+    for k in ("c2p_fail", "atm_reset", "p_floor"):
+        assert do[k] == dg[k]
+    hz.close()
+
+
+def test_papers_energy_variable_is_conserved_to_roundoff_on_the_gpu():
+    """no energy source on a time-independent metric.  Periodic box, smooth space-dependent
+    lapse, shift and 3-metric: the sum of the paper's variable stays put to round-off over 30 substeps in
+    fp64, while sum(sqrt(gamma) tau) of the default form moves (its source is at work)."""
+    from test_oracle_grid import _wavy_metric_workload
+    w = _wavy_metric_workload(40)
+    w1 = dataclasses.replace(w, params={**w.params, "energy_var": 1})
+    a, b = horizon(w, "f64"), horizon(w1, "f64")
+    t0, e0 = a.diagnostics()["sumTau"], b.diagnostics()["sumTau"]
+    a.step(w.dt, 10)
+    b.step(w.dt, 10)
+    t1, e1 = a.diagnostics()["sumTau"], b.diagnostics()["sumTau"]
+    assert abs(e1 - e0) <= 1e-13 * abs(e0), (e0, e1)
+    assert abs(t1 - t0) >= 1e-7 * abs(t0), (t0, t1)
+    a.close()
+    b.close()

@@ -9,6 +9,7 @@ import pytest
 
 import workloads as wl
 from oracle import Oracle, OracleParams
+from parity import oracle_for, rel_l1
 
 
 def make(w, **over):
@@ -327,3 +328,68 @@ def test_hydro_limit_sod_stays_one_dimensional_and_unmagnetised():
     assert np.all(p[5:8] == 0.0) and np.all(p[2:4] == 0.0)
     assert np.array_equal(p[:, 0, 0, :], p[:, 3, 2, :])
     assert p[1].max() > 0.1     # the flow has started
+
+
+# ---- R1b: the paper's own energy variable -sqrt(-g) T^t_t --------------------
+def _wavy_metric_workload(n):
+    """Periodic 2D box with a smooth, time-independent, space-dependent lapse, shift and 3-metric (not a
+    solution of Einstein's equations: the scheme only needs a fixed background) and the Alfven-wave fluid."""
+    import dataclasses
+    w = wl.alfven_wave(n=(n, n, 1))
+    x, _ = wl.centres(n, 0.0, 1.0)
+    X, Y = np.meshgrid(x, x, indexing="xy")
+    X, Y = X[None], Y[None]                       # (nz=1, ny, nx)
+    s, c = np.sin(2 * np.pi * X), np.cos(2 * np.pi * Y)
+    alpha = 1 + 0.1 * s * c
+    beta3 = np.stack([0.05 * c, 0.03 * s, 0.02 * s * c])
+    gamma6 = np.zeros((6,) + alpha.shape)
+    gamma6[0] = 1 + 0.1 * np.cos(2 * np.pi * X)
+    gamma6[1] = 0.03 * s
+    gamma6[3] = 1.0 + 0.05 * c
+    gamma6[5] = 1 + 0.05 * np.sin(2 * np.pi * Y)
+    return dataclasses.replace(w, alpha=alpha, beta3=beta3, gamma6=gamma6)
+
+
+def test_energy_variable_equals_tau_evolution_in_minkowski():
+    """alpha = 1, beta = 0: the variable is tau + D and HLLE is linear in (U, F), so the two evolutions are
+    the same numbers up to rounding."""
+    w = wl.alfven_wave(n=(16, 12, 8))
+    a, b = oracle_for(w), oracle_for(w, energy_var=1)
+    a.substeps(w.dt, 6)
+    b.substeps(w.dt, 6)
+    r = rel_l1(b.get_primitives(), a.get_primitives())
+    assert max(r.values()) <= 1e-12, r
+    Ua, Ub = a.get_conserved(), b.get_conserved()
+    assert np.abs(Ub[4] - (Ua[4] + Ua[0])).max() <= 1e-12 * np.abs(Ub[4]).max()
+
+
+def test_energy_variable_is_conserved_exactly_on_a_fixed_curved_background():
+    """the energy equation's source is T^kappa_lambda Gamma^lambda_{t kappa}, zero for a
+    time-independent metric.  In a periodic box the sum of the paper's variable must then stay constant
+    to round-off (telescoping fluxes, no source), whereas sum(sqrt(gamma) tau) changes through its source."""
+    w = _wavy_metric_workload(24)
+    a, b = oracle_for(w), oracle_for(w, energy_var=1)
+    e0, t0 = b.diagnostics()["sumTau"], a.diagnostics()["sumTau"]
+    a.step(w.dt, 10)
+    b.step(w.dt, 10)
+    e1, t1 = b.diagnostics()["sumTau"], a.diagnostics()["sumTau"]
+    assert abs(e1 - e0) <= 1e-13 * abs(e0), (e0, e1)
+    assert abs(t1 - t0) >= 1e-7 * abs(t0), (t0, t1)       # the tau form has a genuine source here
+    d0 = oracle_for(w, energy_var=1).diagnostics()["sumD"]  # rest mass: source-free in both forms
+    assert abs(b.diagnostics()["sumD"] - d0) <= 1e-13 * abs(d0)
+    assert abs(a.diagnostics()["sumD"] - d0) <= 1e-13 * abs(d0)
+
+
+def test_energy_variable_and_tau_forms_converge_to_each_other():
+    """Both discretise the same equations: their difference is truncation error, second order."""
+    diffs = []
+    for n in (16, 32):
+        w = _wavy_metric_workload(n)
+        nst = 4 * n // 16
+        a, b = oracle_for(w), oracle_for(w, energy_var=1)
+        a.step(w.dt, nst)
+        b.step(w.dt, nst)
+        pa, pb = a.get_primitives(), b.get_primitives()
+        diffs.append(np.abs(pb[4] - pa[4]).mean() / np.abs(pa[4]).mean())
+    assert diffs[0] > 1e-9            # they are different schemes
+    assert diffs[1] < diffs[0] / 2.5, diffs
