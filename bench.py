@@ -325,6 +325,8 @@ def run_gpu(args):
         "cpu_baseline": cpu,
         "state_finite": bool(finite),
         "c2p_fail": d["c2p_fail"], "atm_reset": d["atm_reset"],
+        # hz_diagnostics after the timed steps: conservation sums, div B, CFL number
+        "diagnostics": {**d, "cfl_number": d["max_speed_over_dx"] * w.dt, "steps_run": W + K},
     }
     print(json.dumps(line))
     hz.close()
