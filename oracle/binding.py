@@ -18,7 +18,7 @@ class OracleGrid(C.Structure):
 class OracleParams(C.Structure):
     _fields_ = [("gamma_ad", C.c_double), ("rho_atm", C.c_double), ("p_atm", C.c_double),
                 ("atm_tol", C.c_double), ("cleaning", C.c_int), ("kappa", C.c_double),
-                ("c2p_maxit", C.c_int), ("c2p_tol", C.c_double), ("c2p_scheme", C.c_int), ("energy_var", C.c_int)]
+                ("c2p_maxit", C.c_int), ("c2p_tol", C.c_double), ("c2p_scheme", C.c_int), ("energy_var", C.c_int), ("recon", C.c_int)]
 
     @classmethod
     def default(cls, **kw):
@@ -58,6 +58,8 @@ def lib():
         L.hzo_wavespeed_point.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_int, _dp]
         L.hzo_mc_slope.argtypes = [C.c_double] * 3
         L.hzo_mc_slope.restype = C.c_double
+        L.hzo_ppm_edges.argtypes = [_dp, _dp, _dp]
+        L.hzo_ppm_edges.restype = None
         L.hzo_hlle_point.argtypes = [C.c_int, _dp, _dp, _dp, C.c_double, C.c_int, _dp]
         L.hzo_source_point.argtypes = [_dp, _dp, _dp, C.c_double, _dp]
         L.hzo_default_params.argtypes = [C.POINTER(OracleParams)]
@@ -130,6 +132,12 @@ def wavespeed_point(d, prim9, met10, gamma_ad, cleaning):
 
 def mc_slope(qm, q0, qp):
     return lib().hzo_mc_slope(qm, q0, qp)
+
+
+def ppm_edges(q5):
+    a, b = C.c_double(0), C.c_double(0)
+    lib().hzo_ppm_edges(_p(_arr(q5, 5)), C.byref(a), C.byref(b))
+    return a.value, b.value
 
 
 def hlle_point(d, primL, primR, met10, gamma_ad, cleaning):

@@ -205,6 +205,32 @@ real mc_slope(real qm, real q0, real qp) {
 
 // O5.  HLLE flux through one face: needs only F(u_L), F(u_R) and the speeds.
 // Returns Phi = sqrt(gamma_f) * Fhat.
+// O4b.  PPM ("choice between TVD ... MC limiter, and PPM"; reading R5b): the piecewise
+// parabolic reconstruction of Colella & Woodward on a uniform mesh, without contact steepening and without
+// flattening.  For cell 0 with neighbours q[-2..2] (array q5 = q_{-2}, q_{-1}, q_0, q_1, q_2):
+//   slopes     d_i = the monotonised-central slope of O4 at cells -1, 0, 1
+//   interfaces a_{i+1/2} = q_i + (q_{i+1} - q_i)/2 - (d_{i+1} - d_i)/6
+//   edges      aL = a_{-1/2}, aR = a_{+1/2}, then made monotone:
+//              (aR - q0)(q0 - aL) <= 0                      -> aL = aR = q0   (local extremum: flat)
+//              (aR - aL)(q0 - (aL + aR)/2) >  (aR - aL)^2/6 -> aL = 3 q0 - 2 aR
+//              (aR - aL)(q0 - (aL + aR)/2) < -(aR - aL)^2/6 -> aR = 3 q0 - 2 aL
+void ppm_edges(const real* q5, real* aL, real* aR) {
+  real dm = mc_slope(q5[0], q5[1], q5[2]);
+  real d0 = mc_slope(q5[1], q5[2], q5[3]);
+  real dp = mc_slope(q5[2], q5[3], q5[4]);
+  real l = q5[1] + (q5[2] - q5[1]) / 2 - (d0 - dm) / 6;
+  real r = q5[2] + (q5[3] - q5[2]) / 2 - (dp - d0) / 6;
+  real q0 = q5[2];
+  if ((r - q0) * (q0 - l) <= 0) {
+    l = q0; r = q0;
+  } else {
+    real d = r - l, m = q0 - (l + r) / 2;
+    if (d * m > d * d / 6) l = 3 * q0 - 2 * r;
+    else if (d * m < -(d * d) / 6) r = 3 * q0 - 2 * l;
+  }
+  *aL = l; *aR = r;
+}
+
 void hlle(int d, const Prim& qL, const Prim& qR, const Met& mf, real Gam, int cleaning, real* Phi, int energy_var = 0) {
   Geo geo = geometry(mf);
   real FL[NV], FR[NV], lmL, lpL, lmR, lpR;
@@ -503,7 +529,7 @@ void fill_ghosts(const hzo_ctx* c, std::vector<double>* F, int nf) {
         for (int j = lo[1]; j < hi[1]; j++)
           for (int i = lo[0]; i < hi[0]; i++) {
             int ijk[3] = {i, j, k};
-            for (int s = 1; s <= NG; s++) {
+            for (int s = 1; s <= c->g[d]; s++) {
               int src_lo, src_hi;
               if (c->G.bc[d] == HZO_BC_PERIODIC) {
                 src_lo = ((-s) % nd + nd) % nd;
@@ -541,6 +567,16 @@ void face_flux(const hzo_ctx* c, int d, size_t id, real* Phi) {
   double qL[NV], qR[NV];
   for (int q = 0; q < NV; q++) {
     const double* a = c->P[q].data();
+    if (c->par.recon == 1) {  // O4b: right edge of the cell below the face, left edge of the cell above it
+      real w5[5], lo, hi;
+      for (int t = 0; t < 5; t++) w5[t] = a[id + (size_t)t * s - 2 * s];
+      ppm_edges(w5, &lo, &hi);
+      qL[q] = r_val(hi);
+      for (int t = 0; t < 5; t++) w5[t] = a[id + (size_t)t * s - s];
+      ppm_edges(w5, &lo, &hi);
+      qR[q] = r_val(lo);
+      continue;
+    }
     real sl = mc_slope(a[id - s], a[id], a[id + s]);
     real sr = mc_slope(a[id], a[id + s], a[id + 2 * s]);
     qL[q] = r_val(real(a[id]) + sl / 2);
@@ -755,6 +791,12 @@ int hzo_wavespeed_point(int d, const double* prim9, const double* met10, double 
   return 0;
 }
 double hzo_mc_slope(double qm, double q0, double qp) { return r_val(mc_slope(qm, q0, qp)); }
+void hzo_ppm_edges(const double* q5, double* aL, double* aR) {
+  real w5[5], l, r;
+  for (int t = 0; t < 5; t++) w5[t] = q5[t];
+  ppm_edges(w5, &l, &r);
+  *aL = r_val(l); *aR = r_val(r);
+}
 int hzo_hlle_point(int d, const double* primL, const double* primR, const double* met10, double gamma_ad,
                    int cleaning, double* phi9) {
   real Phi[NV];
@@ -777,7 +819,7 @@ int hzo_default_params(hzo_params* p) {
   p->gamma_ad = 4.0 / 3.0;
   p->rho_atm = 1e-12; p->p_atm = 1e-14; p->atm_tol = 1e-3;
   p->cleaning = 1; p->kappa = 1.0;
-  p->c2p_maxit = 30; p->c2p_tol = 1e-13; p->c2p_scheme = 0; p->energy_var = 0;
+  p->c2p_maxit = 30; p->c2p_tol = 1e-13; p->c2p_scheme = 0; p->energy_var = 0; p->recon = 0;
   return HZO_OK;
 }
 
@@ -787,18 +829,20 @@ int hzo_create(const hzo_grid* G, const hzo_params* par, hzo_ctx** out) {
   const int n3[3] = {G->nx, G->ny, G->nz};
   for (int d = 0; d < 3; d++) {
     if (G->bc[d] != HZO_BC_PERIODIC && G->bc[d] != HZO_BC_OUTFLOW) return HZO_EINVAL;
-    if (n3[d] > 1 && n3[d] < NG) return HZO_EINVAL;
   }
   hzo_ctx* c = new (std::nothrow) hzo_ctx();
   if (!c) return HZO_ENOMEM;
   c->G = *G;
   if (par) c->par = *par; else hzo_default_params(&c->par);
   if (!(c->par.gamma_ad > 1) || c->par.c2p_maxit < 1) { delete c; return HZO_EINVAL; }
+  const int ng = c->par.recon == 1 ? 3 : NG;   // PPM reaches one cell further than MC (reading R16)
+  for (int d = 0; d < 3; d++)
+    if (n3[d] > 1 && n3[d] < ng) { delete c; return HZO_EINVAL; }
   c->h[0] = G->dx; c->h[1] = G->dy; c->h[2] = G->dz;
   c->ncell = 1;
   for (int d = 0; d < 3; d++) {
     c->n[d] = n3[d];
-    c->g[d] = n3[d] > 1 ? NG : 0;
+    c->g[d] = n3[d] > 1 ? ng : 0;
     c->N[d] = c->n[d] + 2 * c->g[d];
     c->ncell *= (size_t)c->N[d];
   }

@@ -46,6 +46,7 @@ typedef struct {
   int    c2p_scheme;       /* 0: Newton on Z (O8); 1: Newton on (Z, v^2) (O8b)       */
   int    energy_var;       /* 0: evolve sqrt(gamma) tau (R1); 1: the paper's          */
                            /* -sqrt(-g) T^t_t (R1b): slot 4 of U, source-free        */
+  int    recon;            /* 0: MC-limited linear (O4); 1: PPM (O4b), 3 ghost layers */
 } hzo_params;
 
 typedef struct {
@@ -69,6 +70,7 @@ int    hzo_flux_point(int d, const double* prim9, const double* met10, double ga
 int    hzo_wavespeed_point(int d, const double* prim9, const double* met10, double gamma_ad,
                            int cleaning, double* lam_minus_plus);
 double hzo_mc_slope(double qm, double q0, double qp);
+void hzo_ppm_edges(const double* q5, double* aL, double* aR);
 /* HLLE flux Phi = sqrt(gamma_f) * Fhat through one face with face metric met10 */
 int    hzo_hlle_point(int d, const double* primL, const double* primR, const double* met10,
                       double gamma_ad, int cleaning, double* phi9);

@@ -393,3 +393,45 @@ def test_energy_variable_and_tau_forms_converge_to_each_other():
         diffs.append(np.abs(pb[4] - pa[4]).mean() / np.abs(pa[4]).mean())
     assert diffs[0] > 1e-9            # they are different schemes
     assert diffs[1] < diffs[0] / 2.5, diffs
+
+
+# ---- O4b: PPM on the grid (reading R5b) ------------------------------------------------------
+def test_ppm_keeps_invariants_and_beats_mc_on_the_smooth_wave():
+    """With PPM (3 ghost layers) the scheme must keep what the pins fix for MC -- uniform state on a constant
+    curved metric is a fixed point, D, S, tau, B conserved to round-off in the periodic Minkowski box -- and on
+    the smooth Alfven wave (closed-form solution: the initial data after one period) its error must be well
+    below MC's at the same resolution and fall with resolution."""
+    # fixed point
+    n = (8, 6, 5)
+    a, b, g = wl.constant_metric(n)
+    w = wl.alfven_wave(n=n)
+    prim = np.zeros_like(w.prim8)
+    prim[0], prim[4] = 1.3, 0.7
+    prim[1], prim[2], prim[3] = 0.2, -0.1, 0.15
+    prim[5], prim[6], prim[7] = 0.3, 0.2, -0.4
+    import dataclasses
+    wu = dataclasses.replace(w, alpha=a, beta3=b, gamma6=g, prim8=prim)
+    o = oracle_for(wu, recon=1)
+    o.step(w.dt, 3)
+    assert np.abs(o.get_primitives() - prim).max() <= 1e-13
+    # conservation
+    w = wl.alfven_wave(n=(16, 12, 10))
+    o = oracle_for(w, recon=1)
+    d0 = o.diagnostics()
+    o.step(w.dt, 10)
+    d1 = o.diagnostics()
+    for k in ("sumD", "sumTau", "sumBx", "sumBy", "sumBz"):
+        assert abs(d1[k] - d0[k]) <= 1e-13 * max(abs(d0[k]), 1.0), k
+    for k in ("sumSx", "sumSy", "sumSz"):
+        assert abs(d1[k] - d0[k]) <= 1e-13
+    # accuracy on the 1D wave over a quarter period
+    errs = {}
+    for recon in (0, 1):
+        for nx in (32, 64):
+            w = wl.alfven_wave(nx, direction="x")
+            nst = w.nsteps
+            o = oracle_for(w, recon=recon)
+            o.step(w.dt, nst)
+            errs[(recon, nx)] = np.abs(o.get_primitives()[6] - w.prim8[6]).mean()
+    assert errs[(1, 32)] < 0.6 * errs[(0, 32)] and errs[(1, 64)] < 0.6 * errs[(0, 64)], errs
+    assert errs[(1, 64)] < errs[(1, 32)] / 3.0, errs

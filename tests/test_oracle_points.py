@@ -342,3 +342,37 @@ def test_two_unknown_scheme_is_a_different_iteration():
         it2 = ob.con2prim_point(w, m, par2)[2]
         differ += it1 != it2
     assert differ > 30, differ
+
+
+# ---- O4b: PPM edge values (reading R5b) ---------------------------------------------------
+def test_ppm_edges_closed_forms():
+    """Pins of the piecewise parabolic reconstruction: exact on linear data; the unlimited interface value
+    a_{i+1/2} = q_i + (q_{i+1} - q_i)/2 - (d_{i+1} - d_i)/6 when no slope is clipped; flat at a local extremum;
+    edges bounded by the three cells they come from; and Colella & Woodward's no-interior-extremum condition
+    |aR - aL| >= 6 |q0 - (aL + aR)/2| after limiting."""
+    # linear data: edges are the linear interpolants
+    for slope in (0.3, -2.0):
+        q5 = [1.0 + slope * i for i in range(-2, 3)]
+        aL, aR = ob.ppm_edges(q5)
+        assert abs(aL - (1.0 - slope / 2)) < 1e-15 and abs(aR - (1.0 + slope / 2)) < 1e-15
+    # unlimited interface value: (7 (q_i + q_{i+1}) - (q_{i-1} + q_{i+2})) / 12 when no slope is clipped
+    q5 = [0.0, 1.0, 2.1, 3.3, 4.6]                 # monotone, gently curved: MC slopes are the centred ones
+    aL, aR = ob.ppm_edges(q5)
+    # slopes: d_{-1} = (2.1 - 0)/2, d_0 = (3.3 - 1)/2, d_1 = (4.6 - 2.1)/2
+    dm, d0, dp = 1.05, 1.15, 1.25
+    assert abs(aL - (1.0 + 0.55 - (d0 - dm) / 6)) < 1e-15
+    assert abs(aR - (2.1 + 0.6 - (dp - d0) / 6)) < 1e-15
+    # local extremum: flat
+    assert ob.ppm_edges([0.0, 1.0, 2.0, 1.0, 0.0]) == (2.0, 2.0)
+    # steep one-sided profile: the parabola would overshoot, the monotonisation pulls one edge in
+    aL, aR = ob.ppm_edges([0.0, 0.0, 0.1, 1.0, 1.0])
+    assert 0.0 <= aL <= 0.1 <= aR <= 1.0
+    # the parabola through (aL, q0 as mean, aR) has no interior extremum after limiting:
+    # |aR - aL| >= 6 |q0 - (aL + aR)/2|  (Colella & Woodward's condition)
+    rng = np.random.default_rng(7)
+    for _ in range(2000):
+        q5 = rng.normal(size=5).cumsum() if rng.random() < 0.5 else rng.normal(size=5)
+        aL, aR = ob.ppm_edges(q5)
+        lo, hi = min(q5[1:4]), max(q5[1:4])
+        assert lo - 1e-14 <= aL <= hi + 1e-14 and lo - 1e-14 <= aR <= hi + 1e-14
+        assert abs(aR - aL) * (1 + 1e-12) + 1e-15 >= 6 * abs(q5[2] - 0.5 * (aL + aR))
