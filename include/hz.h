@@ -74,6 +74,8 @@ typedef struct {
                           /* own variable -sqrt(-g) T^t_t = sqrt(gamma)[alpha(tau+D) - beta^j S_j]   */
                           /* (PAPER.md:54, 60), which has no source on a fixed metric; hz_get_conserved */
                           /* and hz_diag.sumTau then carry that variable.                            */
+  int    recon;           /* reconstruction: 0 TVD with the MC limiter (2 ghost layers), */
+                          /* 1 PPM (3 ghost layers; an active axis then needs at least 3 cells)       */
 } hz_params;
 
 /* Global reductions, all accumulated in fp64. */
@@ -87,7 +89,7 @@ typedef struct {
 } hz_diag;
 
 /* Fill *p with the defaults: Gamma = 4/3, atmosphere 1e-12 / 1e-14, atm_tol 1e-3, cleaning on,
- * kappa = 1, 30 Newton iterations, c2p_tol = 0 (dtype default), c2p_scheme = 0, energy_var = 0.  HZ_EINVAL if p is NULL. */
+ * kappa = 1, 30 Newton iterations, c2p_tol = 0 (dtype default), c2p_scheme = 0, energy_var = 0, recon = 0.  HZ_EINVAL if p is NULL. */
 int hz_default_params(hz_params* p);
 
 /* Bytes of device memory one context of this grid and dtype needs (all resident fields: metric,
@@ -142,7 +144,7 @@ int hz_diagnostics(hz_ctx* ctx, hz_diag* out);
  * kernel, every substep; here the transfer is device-to-device and the caller's: NCCL send/recv over
  * NVLink between processes, or a plain copy between contexts of one process).  `which` selects the
  * primitives (9 fields) or the metric (10 fields); `side` 0 = low z, 1 = high z.
- * hz_halo_pack copies the NG = 2 interior planes next to that side -- whole padded planes, so the x and y
+ * hz_halo_pack copies the NG interior planes next to that side (NG = 2 with MC, 3 with PPM) -- whole padded planes, so the x and y
  * ghost columns travel too -- into `device_buf` (hz_halo_bytes bytes, DEVICE memory, context dtype);
  * hz_halo_unpack writes such a buffer into the ghost planes of that side.  A slab's low-side buffer
  * goes to the high-side ghosts of the slab below it and vice versa.  Both are asynchronous on the context

@@ -26,7 +26,7 @@ class HzGrid(C.Structure):
 class HzParams(C.Structure):
     _fields_ = [("gamma_ad", C.c_double), ("rho_atm", C.c_double), ("p_atm", C.c_double), ("atm_tol", C.c_double),
                 ("cleaning", C.c_int), ("kappa", C.c_double), ("c2p_maxit", C.c_int), ("c2p_tol", C.c_double),
-                ("c2p_scheme", C.c_int), ("energy_var", C.c_int)]
+                ("c2p_scheme", C.c_int), ("energy_var", C.c_int), ("recon", C.c_int)]
 
     @classmethod
     def default(cls, **kw):

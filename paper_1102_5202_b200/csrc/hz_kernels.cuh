@@ -55,11 +55,11 @@ __global__ void k_fill_ghosts(Layout L, T* __restrict__ F, int nf) {
   for (int f = 0; f < nf; f++) F[f * L.fs + dst] = F[f * L.fs + src];
 }
 
-// ---- hz_halo_pack / hz_halo_unpack: NG whole padded z planes of nf fields <-> one contiguous buffer ----
+// ---- hz_halo_pack / hz_halo_unpack: ng whole padded z planes of nf fields <-> one contiguous buffer ----
 // k0: first storage plane; buffer layout [field][plane][y][x] with the padded extents of the context.
 template <typename T>
 __global__ void k_halo_copy(Layout L, T* __restrict__ F, int nf, int k0, T* __restrict__ buf, int unpack) {
-  const long long per = (long long)NG * L.sz, tot = per * nf;
+  const long long per = (long long)L.ng * L.sz, tot = per * nf;
   for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < tot; e += (long long)gridDim.x * blockDim.x) {
     const long long f = e / per, r = e - f * per;
     T* cell = F + f * L.fs + (long long)k0 * L.sz + r;

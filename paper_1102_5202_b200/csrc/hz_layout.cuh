@@ -21,7 +21,8 @@ __host__ __device__ inline int bc_side(int bc, int side) {
 
 struct Layout {
   int n[3];        // interior cells per axis
-  int g[3];        // ghost layers per side (NG on active axes, 0 on one-cell axes)
+  int ng;          // ghost layers of an active axis: 2 (MC) or 3 (PPM)
+  int g[3];        // ghost layers per side (ng on active axes, 0 on one-cell axes)
   int N[3];        // padded logical extent n + 2g
   int ox;          // x offset of interior cell 0 inside a row
   int pitch;       // row length in elements

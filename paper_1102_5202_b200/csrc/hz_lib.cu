@@ -19,27 +19,28 @@ namespace {
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline size_t elem_size(int dtype) { return dtype == HZ_F64 ? 8 : 4; }
 
-bool grid_ok(const hz_grid* G) {
+bool grid_ok(const hz_grid* G, int ng = NG) {
   if (!G) return false;
   const int n3[3] = {G->nx, G->ny, G->nz};
   if (!(G->dx > 0) || !(G->dy > 0) || !(G->dz > 0)) return false;
   if (!std::isfinite(G->dx) || !std::isfinite(G->dy) || !std::isfinite(G->dz)) return false;
   for (int d = 0; d < 3; d++) {
     if (n3[d] < 1) return false;
-    if (n3[d] > 1 && n3[d] < NG) return false;
+    if (n3[d] > 1 && n3[d] < ng) return false;
     const bool ext = G->bc[d] >= HZ_BC_EXTERNAL && G->bc[d] <= HZ_BC_OUTFLOW_EXTERNAL;
-    if (G->bc[d] != HZ_BC_PERIODIC && G->bc[d] != HZ_BC_OUTFLOW && !(ext && d == 2 && n3[d] >= NG)) return false;
+    if (G->bc[d] != HZ_BC_PERIODIC && G->bc[d] != HZ_BC_OUTFLOW && !(ext && d == 2 && n3[d] >= ng)) return false;
   }
   return true;
 }
 
-Layout make_layout(const hz_grid& G, int dtype) {
+Layout make_layout(const hz_grid& G, int dtype, int ng) {
   Layout L;
+  L.ng = ng;
   const int n3[3] = {G.nx, G.ny, G.nz};
   const int ae = (int)(128 / elem_size(dtype));  // elements per 128 bytes
   for (int d = 0; d < 3; d++) {
     L.n[d] = n3[d];
-    L.g[d] = n3[d] > 1 ? NG : 0;
+    L.g[d] = n3[d] > 1 ? ng : 0;
     L.N[d] = L.n[d] + 2 * L.g[d];
     L.bc[d] = G.bc[d];
   }
@@ -242,26 +243,26 @@ int set_prims_t(hz_ctx* c, const void* prim8) {
   return flag ? HZ_EINVAL : HZ_OK;
 }
 
-template <typename T>
-int substep_t(hz_ctx* c, double dt) {
+template <typename T, int R>
+int substep_tr(hz_ctx* c, double dt) {
   const Layout& L = c->L;
   const Par<T> par = make_par<T>(c);
   const int st = c->stage;
   const T* Uin = c->U<T>(c->cur);
   T* Uout = st == 0 ? c->U<T>(1 - c->cur) : c->U<T>(c->cur);
   const T* U0 = st == 0 ? Uin : c->U<T>(c->u0);
-  using G = TileGeom<T>;
+  using G = TileGeom<T, R>;
   const int ntx = (L.n[0] + G::TX - 1) / G::TX, nty = (L.n[1] + G::TY - 1) / G::TY, ntz = (L.n[2] + G::TZ - 1) / G::TZ;
   const long long ntiles = (long long)ntx * nty * ntz;
   const unsigned grid = (unsigned)(ntiles < c->nsm ? ntiles : c->nsm);  // persistent: one block per SM
   {
     ProfScope ps(c, K_SUBSTEP);
     if (sizeof(T) == 4 && c->dtype == HZ_F32_F64)  // fp32 storage and faces, fp64 flux difference / RK / con2prim
-      k_substep<float, double><<<grid, G::NT, G::SMEM, c->stream>>>(
+      k_substep<float, double, R><<<grid, G::NT, G::SMEM, c->stream>>>(
           c->tmP[c->pcur], c->tmM, L, make_par<float>(c), make_par<double>(c), (const float*)Uin, (const float*)U0,
           (float*)Uout, (float*)c->P<T>(1 - c->pcur), st, dt, c->counters(), ntx, nty, (int)ntiles);
     else
-      k_substep<T, T><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, par, Uin, U0, Uout,
+      k_substep<T, T, R><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, par, Uin, U0, Uout,
                                                             c->P<T>(1 - c->pcur), st, (T)dt, c->counters(), ntx, nty,
                                                             (int)ntiles);
   }
@@ -271,13 +272,17 @@ int substep_t(hz_ctx* c, double dt) {
   c->stage = (st + 1) % 3;
   return HZ_OK;
 }
+template <typename T>
+int substep_t(hz_ctx* c, double dt) {   // R: reconstruction (0 MC, 1 PPM) -- tile shape and ghost width follow it
+  return c->par.recon == 1 ? substep_tr<T, 1>(c, dt) : substep_tr<T, 0>(c, dt);
+}
 
 // Tensor map of a padded SoA field set as a 4D array (x, y, z, field) with the staging box of k_substep.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 template <typename T>
-int make_tensor_map(const Layout& L, void* base, int nfields, int by, int bz, CUtensorMap* out) {
+int make_tensor_map(const Layout& L, void* base, int nfields, int bx, int by, int bz, CUtensorMap* out) {
   static EncodeTiledFn encode = nullptr;
   if (!encode) {
     void* fn = nullptr;
@@ -288,31 +293,34 @@ int make_tensor_map(const Layout& L, void* base, int nfields, int by, int bz, CU
     }
     encode = (EncodeTiledFn)fn;
   }
-  using G = TileGeom<T>;
   const cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.N[1], (cuuint64_t)L.N[2], (cuuint64_t)nfields};
   const cuuint64_t strides[3] = {(cuuint64_t)L.pitch * sizeof(T), (cuuint64_t)L.sz * sizeof(T),
                                  (cuuint64_t)L.fs * sizeof(T)};
-  const cuuint32_t box[4] = {(cuuint32_t)G::BX, (cuuint32_t)by, (cuuint32_t)bz, (cuuint32_t)nfields};
+  const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz, (cuuint32_t)nfields};
   const cuuint32_t es[4] = {1, 1, 1, 1};
   const CUresult r = encode(out, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4,
                             base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? HZ_OK : HZ_ECUDA;
 }
-template <typename T>
-int make_maps_t(hz_ctx* c) {
-  using G = TileGeom<T>;
+template <typename T, int R>
+int make_maps_tr(hz_ctx* c) {
+  using G = TileGeom<T, R>;
   int rc;
   for (int w = 0; w < 2; w++)
-    if ((rc = make_tensor_map<T>(c->L, c->P<T>(w), NV, G::BY, G::BZ, &c->tmP[w]))) return rc;
-  if ((rc = make_tensor_map<T>(c->L, c->met<T>(), NM, G::MY, G::MZ, &c->tmM))) return rc;
-  if (cudaFuncSetAttribute(k_substep<T, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM) != cudaSuccess ||
-      cudaFuncSetAttribute(k_substep<float, double>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)TileGeom<float>::SMEM) != cudaSuccess) {
+    if ((rc = make_tensor_map<T>(c->L, c->P<T>(w), NV, G::BX, G::BY, G::BZ, &c->tmP[w]))) return rc;
+  if ((rc = make_tensor_map<T>(c->L, c->met<T>(), NM, G::BX, G::MY, G::MZ, &c->tmM))) return rc;
+  if (cudaFuncSetAttribute(k_substep<T, T, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(k_substep<float, double, R>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)TileGeom<float, R>::SMEM) != cudaSuccess) {
     cudaGetLastError();
     return HZ_ECUDA;
   }
   return HZ_OK;
+}
+template <typename T>
+int make_maps_t(hz_ctx* c) {
+  return c->par.recon == 1 ? make_maps_tr<T, 1>(c) : make_maps_tr<T, 0>(c);
 }
 
 // Run a kernel result out to the user: directly if `dst` is a device pointer, else through staging.
@@ -381,7 +389,7 @@ template <typename T>
 int halo_copy_t(hz_ctx* c, int which, int k0, void* buf, int unpack) {
   const int nf = which == HZ_HALO_PRIM ? NV : NM;
   T* F = which == HZ_HALO_PRIM ? c->P<T>(c->pcur) : c->met<T>();
-  const long long tot = (long long)nf * NG * c->L.sz;
+  const long long tot = (long long)nf * c->L.ng * c->L.sz;
   const unsigned nb = (unsigned)((tot + 255) / 256 < 4736 ? (tot + 255) / 256 : 4736);
   k_halo_copy<T><<<nb, 256, 0, c->stream>>>(c->L, F, nf, k0, (T*)buf, unpack);
   HZ_LAUNCHED(c);
@@ -399,13 +407,14 @@ int hz_default_params(hz_params* p) {
   p->gamma_ad = 4.0 / 3.0;
   p->rho_atm = 1e-12; p->p_atm = 1e-14; p->atm_tol = 1e-3;
   p->cleaning = 1; p->kappa = 1.0;
-  p->c2p_maxit = 30; p->c2p_tol = 0.0; p->c2p_scheme = 0; p->energy_var = 0;
+  p->c2p_maxit = 30; p->c2p_tol = 0.0; p->c2p_scheme = 0; p->energy_var = 0; p->recon = 0;
   return HZ_OK;
 }
 
 int hz_state_bytes(const hz_grid* grid, int dtype, size_t* bytes) {
   if (!grid_ok(grid) || !bytes || (dtype != HZ_F32 && dtype != HZ_F64 && dtype != HZ_F32_F64)) return HZ_EINVAL;
-  *bytes = make_plan(make_layout(*grid, dtype), dtype).total;
+  // the size of the larger layout (3 ghost layers, PPM): enough for either reconstruction
+  *bytes = make_plan(make_layout(*grid, dtype, 3), dtype).total;
   return HZ_OK;
 }
 
@@ -415,14 +424,16 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
   if (!grid_ok(grid) || (dtype != HZ_F32 && dtype != HZ_F64 && dtype != HZ_F32_F64)) return HZ_EINVAL;
   hz_params par;
   if (params) par = *params; else hz_default_params(&par);
-  if (!(par.gamma_ad > 1) || par.c2p_maxit < 1 || (par.c2p_scheme != 0 && par.c2p_scheme != 1) || (par.energy_var != 0 && par.energy_var != 1) || !(par.rho_atm > 0) || !(par.p_atm > 0) || !(par.atm_tol >= 0))
+  if (!(par.gamma_ad > 1) || par.c2p_maxit < 1 || (par.c2p_scheme != 0 && par.c2p_scheme != 1) || (par.energy_var != 0 && par.energy_var != 1) || (par.recon != 0 && par.recon != 1) || !(par.rho_atm > 0) || !(par.p_atm > 0) || !(par.atm_tol >= 0))
     return HZ_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return HZ_ECUDA; }
   hz_ctx* c = new (std::nothrow) hz_ctx();
   if (!c) return HZ_ENOMEM;
   c->G = *grid; c->par = par; c->dtype = dtype;
-  c->L = make_layout(*grid, dtype);
+  const int ng = par.recon == 1 ? 3 : NG;
+  if (!grid_ok(grid, ng)) { delete c; return HZ_EINVAL; }
+  c->L = make_layout(*grid, dtype, ng);
   c->plan = make_plan(c->L, dtype);
   c->stream = 0;
   c->own = device_buffer == nullptr;
@@ -532,7 +543,7 @@ int hz_diagnostics(hz_ctx* c, hz_diag* out) {
 // ---- slab decomposition along z: ghost planes of an external side ----
 int hz_halo_bytes(const hz_ctx* c, int which, size_t* bytes) {
   if (!c || !bytes || (which != HZ_HALO_PRIM && which != HZ_HALO_METRIC) || c->L.g[2] == 0) return HZ_EINVAL;
-  *bytes = (size_t)(which == HZ_HALO_PRIM ? NV : NM) * NG * (size_t)c->L.sz * elem_size(c->dtype);
+  *bytes = (size_t)(which == HZ_HALO_PRIM ? NV : NM) * c->L.ng * (size_t)c->L.sz * elem_size(c->dtype);
   return HZ_OK;
 }
 
@@ -541,7 +552,7 @@ int hz_halo_pack(hz_ctx* c, int which, int side, void* device_buf) {
   if (rc) return rc;
   if (!device_buf || !is_device_ptr(device_buf)) return HZ_EINVAL;
   // the NG interior planes next to that side: they become the neighbour's ghost planes
-  const int k0 = side == 0 ? c->L.g[2] : c->L.g[2] + c->L.n[2] - NG;
+  const int k0 = side == 0 ? c->L.g[2] : c->L.g[2] + c->L.n[2] - c->L.ng;
   return HZ_DISPATCH(c, halo_copy_t, c, which, k0, device_buf, 0);
 }
 

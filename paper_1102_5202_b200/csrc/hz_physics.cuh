@@ -159,6 +159,36 @@ __device__ __forceinline__ double mc_slope<double>(double qm, double q0, double 
   return s;
 }
 
+// PPM (O4b / R5b): Colella-Woodward edge values on a uniform mesh, built on the
+// monotonised-central slopes above, made monotone, without contact steepening or flattening.
+// Edges of the cell with value q0, from the interface values l, r on its two sides.
+template <typename T>
+__device__ __forceinline__ void ppm_monotone(T q0, T& l, T& r) {
+  if ((r - q0) * (q0 - l) <= 0) {
+    l = q0; r = q0;
+  } else {
+    const T d = r - l, m = q0 - (l + r) * T(0.5);
+    if (d * m > d * d * T(1.0 / 6.0)) l = 3 * q0 - 2 * r;
+    else if (d * m < -(d * d) * T(1.0 / 6.0)) r = 3 * q0 - 2 * l;
+  }
+}
+// The two states of the face between cells 0 and 1 from the six cells -2 .. 3:
+// qL = right edge of cell 0, qR = left edge of cell 1.
+template <typename T>
+__device__ __forceinline__ void ppm_face(T qm2, T qm1, T q0, T q1, T q2, T q3, T& qL, T& qR) {
+  const T dm1 = mc_slope(qm2, qm1, q0), d0 = mc_slope(qm1, q0, q1);
+  const T d1 = mc_slope(q0, q1, q2), d2 = mc_slope(q1, q2, q3);
+  const T s6 = T(1.0 / 6.0);
+  T am = qm1 + (q0 - qm1) * T(0.5) - (d0 - dm1) * s6;   // interface -1/2
+  T ac = q0 + (q1 - q0) * T(0.5) - (d1 - d0) * s6;      // interface +1/2: the face
+  T ap = q1 + (q2 - q1) * T(0.5) - (d2 - d1) * s6;      // interface +3/2
+  T l0 = am, r0 = ac, l1 = ac, r1 = ap;
+  ppm_monotone(q0, l0, r0);
+  ppm_monotone(q1, l1, r1);
+  qL = r0;
+  qR = l1;
+}
+
 // ---- R1b: the paper's energy variable -------------------------------------------
 // -sqrt(-g) T^t_t = sqrt(gamma) [alpha (tau + D) - beta^j S_j]; source-free on a fixed metric.  The two maps
 // swap slot 4 of an undensitised (D, S_j, tau, ...) vector -- or, the map being linear, of a coordinate-flux

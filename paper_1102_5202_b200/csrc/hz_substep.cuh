@@ -28,18 +28,23 @@ namespace hz {
 
 // Tile shape, threads per block (= cells per tile) and x halo of the staged boxes.  TMA wants the first
 // element of every box row on a 16-byte boundary, so the x halo is 16 bytes: 2 doubles or 4 floats.
-template <typename T> struct Tile;
-template <> struct Tile<double> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = 256, HX = 2; };
-template <> struct Tile<float> { static constexpr int TX = 16, TY = 8, TZ = 4, NT = 512, HX = 4; };
+// R = 0: MC-limited linear reconstruction, 2 ghost layers; R = 1: PPM, 3 ghost layers (R5, R5b, R16).
+// PPM's wider halo makes the staged boxes bigger, so its tiles are smaller.
+template <typename T, int R> struct Tile;
+template <> struct Tile<double, 0> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = 256, HX = 2; };
+template <> struct Tile<float, 0> { static constexpr int TX = 16, TY = 8, TZ = 4, NT = 512, HX = 4; };
+template <> struct Tile<double, 1> { static constexpr int TX = 8, TY = 4, TZ = 4, NT = 128, HX = 4; };
+template <> struct Tile<float, 1> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = 256, HX = 4; };
 
-template <typename T>
+template <typename T, int R>
 struct TileGeom {
-  static constexpr int TX = Tile<T>::TX, TY = Tile<T>::TY, TZ = Tile<T>::TZ, NT = Tile<T>::NT, HX = Tile<T>::HX;
+  static constexpr int NG = R == 1 ? 3 : 2;  // ghost layers = halo of the staged primitives
+  static constexpr int TX = Tile<T, R>::TX, TY = Tile<T, R>::TY, TZ = Tile<T, R>::TZ, NT = Tile<T, R>::NT, HX = Tile<T, R>::HX;
   static constexpr int NC = TX * TY * TZ;
   static constexpr int NFX = (TX + 1) * TY * TZ, NFY = TX * (TY + 1) * TZ, NFZ = TX * TY * (TZ + 1);
   static constexpr int NF = NFX + NFY + NFZ;
-  static constexpr int WX = NFX / 32, WY = NFY / 32, WZ = NFZ / 32;  // warp tasks per direction
-  static_assert(NFX % 32 == 0 && NFY % 32 == 0 && NFZ % 32 == 0, "face lists must split into whole warps");
+  static constexpr int WX = (NFX + 31) / 32, WY = (NFY + 31) / 32, WZ = (NFZ + 31) / 32;  // warp items per direction
+  // (the last item of a direction may be partly empty)
   static_assert(NC == NT, "phase 2 maps one cell to one thread");
   static_assert(TY % 4 == 0, "the row swizzle permutes groups of four rows");
   static_assert(HX >= NG && (HX * sizeof(T)) % 16 == 0, "x halo: at least NG cells and 16-byte box rows starts");
@@ -178,10 +183,10 @@ __device__ __forceinline__ void state_flux0(const T* q, const T* m, const T* gi0
 // sPc / sMc: staged primitives / metric at the cell on the MINUS side of the face (field 0);
 // sp / sm: element stride of axis d inside the two boxes.
 // Phi comes out in the sweep frame: Phi[1+a] belongs to S_{(d+a)%3}, Phi[5+a] to B^{(d+a)%3}.
-template <typename T>
+template <typename T, int R>
 __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T* __restrict__ sMc, int sp, int sm,
                                               int d, const Par<T>& par, T* Phi) {
-  using G = TileGeom<T>;
+  using G = TileGeom<T, R>;
   // face metric: mean of the two cells (R8), components rotated into the sweep frame
   T mf[NM];
   mf[AL] = T(0.5) * (sMc[0] + sMc[sm]);
@@ -210,9 +215,13 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
   for (int q = 0; q < NV; q++) {
     const int f = (q >= UX && q <= UZ) ? UX + rot3(d, q - UX) : ((q >= BX && q <= BZ) ? BX + rot3(d, q - BX) : q);
     const T* a = sPc + f * G::PFS;
-    const T qm = a[-sp], q0 = a[0], q1 = a[sp], q2 = a[2 * sp];
-    qL[q] = q0 + T(0.5) * mc_slope(qm, q0, q1);
-    qR[q] = q1 - T(0.5) * mc_slope(q0, q1, q2);
+    if (R == 1) {  // PPM (O4b): right edge of the cell below the face, left edge of the cell above it
+      ppm_face(a[-2 * sp], a[-sp], a[0], a[sp], a[2 * sp], a[3 * sp], qL[q], qR[q]);
+    } else {
+      const T qm = a[-sp], q0 = a[0], q1 = a[sp], q2 = a[2 * sp];
+      qL[q] = q0 + T(0.5) * mc_slope(qm, q0, q1);
+      qR[q] = q1 - T(0.5) * mc_slope(q0, q1, q2);
+    }
   }
   qL[RHO] = max_(qL[RHO], par.rho_atm); qL[PR] = max_(qL[PR], par.p_atm);
   qR[RHO] = max_(qR[RHO], par.rho_atm); qR[PR] = max_(qR[PR], par.p_atm);
@@ -241,10 +250,10 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
 
 // ---- a6 from the staged metric: centred differences, fluid and cleaning sources at a cell ----------
 // sMc: staged metric at the cell (field 0).  Same arithmetic as add_sources (hz_kernels.cuh).
-template <typename T>
+template <typename T, int R>
 __device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __restrict__ sMc, const T* m, const T* q,
-                                                   const Par<T>& par, const T* gi, T sq, T* R) {
-  using G = TileGeom<T>;
+                                                   const Par<T>& par, const T* gi, T sq, T* Rs) {
+  using G = TileGeom<T, R>;
   T dm[3][NM];
   T dQ[3] = {0, 0, 0};  // sum_j d_j(alpha sqrt(gamma) gamma^{kj})
   T dRb = 0;            // sum_j d_j(sqrt(gamma) beta^j)
@@ -272,17 +281,17 @@ __device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __r
       dRb += (sp * mp[BEX + d] - sn * mm[BEX + d]) * i2h;
     }
   }
-  fluid_source(q, m, dm, par, gi, sq, R);
+  fluid_source(q, m, dm, par, gi, sq, Rs);
   if (par.cleaning) {  // cleaning sources (R14), not multiplied by alpha
 #pragma unroll
     for (int k = 0; k < 3; k++) {
       const T adv = q[BX] * dm[0][BEX + k] + q[BY] * dm[1][BEX + k] + q[BZ] * dm[2][BEX + k];
-      R[5 + k] += -sq * adv + q[PSI] * dQ[k];
+      Rs[5 + k] += -sq * adv + q[PSI] * dQ[k];
     }
     const T Bda = q[BX] * dm[0][AL] + q[BY] * dm[1][AL] + q[BZ] * dm[2][AL];
-    R[8] += sq * Bda - q[PSI] * dRb - m[AL] * par.kappa * sq * q[PSI];
+    Rs[8] += sq * Bda - q[PSI] * dRb - m[AL] * par.kappa * sq * q[PSI];
   } else {
-    R[8] = 0;
+    Rs[8] = 0;
   }
 }
 
@@ -291,7 +300,7 @@ template <typename T>
 __device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __restrict__ Pout, int i, int j, int k,
                                                         const T* q) {
   const int c3[3] = {i, j, k};
-  int dst[3][3], cnt[3];
+  int dst[3][4], cnt[3];   // the cell itself and up to 3 images per axis
   bool plain = true;
 #pragma unroll
   for (int d = 0; d < 3; d++) {
@@ -300,11 +309,16 @@ __device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __re
     cnt[d] = 1;
     if (L.g[d]) {
       if (L.bc[d] == 0) {  // periodic wrap
-        if (c < NG) dst[d][cnt[d]++] = c + n;
-        if (c >= n - NG) dst[d][cnt[d]++] = c - n;
+        if (c < L.ng) dst[d][cnt[d]++] = c + n;
+        if (c >= n - L.ng) dst[d][cnt[d]++] = c - n;
       } else {             // zero gradient: the edge cell fills its ghost layers; external sides are left alone
-        if (c == 0 && bc_side(L.bc[d], 0) == 1) { dst[d][1] = -1; dst[d][2] = -2; cnt[d] = 3; }
-        else if (c == n - 1 && bc_side(L.bc[d], 1) == 1) { dst[d][1] = n; dst[d][2] = n + 1; cnt[d] = 3; }
+        if (c == 0 && bc_side(L.bc[d], 0) == 1) {
+          for (int t = 1; t <= L.ng; t++) dst[d][t] = -t;
+          cnt[d] = 1 + L.ng;
+        } else if (c == n - 1 && bc_side(L.bc[d], 1) == 1) {
+          for (int t = 1; t <= L.ng; t++) dst[d][t] = n - 1 + t;
+          cnt[d] = 1 + L.ng;
+        }
       }
     }
     plain = plain && cnt[d] == 1;
@@ -346,16 +360,17 @@ __device__ __forceinline__ int cdiv(int n) {
 
 // ---- the work items of phase 1 ----------------------------------------------------------------------
 // Face item: 32 consecutive faces of one direction -> Phi into sF.
-template <typename T>
+template <typename T, int R>
 __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, const T* sP, const T* sM, T* sF, int task,
                                           int lane, int x0, int y0, int z0) {
-  using G = TileGeom<T>;
+  using G = TileGeom<T, R>;
   int d = (task >= G::WX) + (task >= G::WX + G::WY);
   // keep ONE copy of the face-flux body: hide the value of d so the compiler does not clone it per axis
   asm volatile("" : "+r"(d));
-  const int off = d == 0 ? 0 : (d == 1 ? G::NFX : G::NFX + G::NFY);
-  const int f = task * 32 - off + lane;
+  const int off = d == 0 ? 0 : (d == 1 ? G::NFX : G::NFX + G::NFY);                 // first face of d in sF
+  const int f = (task - (d == 0 ? 0 : (d == 1 ? G::WX : G::WX + G::WY))) * 32 + lane;  // face number within d
   if (L.g[d] == 0) return;
+  if (f >= (d == 0 ? G::NFX : (d == 1 ? G::NFY : G::NFZ))) return;                     // partly empty last item
   // face coordinates inside the tile: f = (c * e1 + b) * e0 + a with e0 = TX (+1 for x faces),
   // e1 = TY (+1 for y faces); the quotients by multiply-shift (d is a run-time value here)
   const int e0 = G::TX + (d == 0), e1 = G::TY + (d == 1);
@@ -369,10 +384,10 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
   if (!valid) return;
   const int sp = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::BY);
   const int sm = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::MY);
-  const T* sPc = sP + ((c + NG) * G::BY + (b + NG)) * G::BX + (a + G::HX) - sp;
+  const T* sPc = sP + ((c + G::NG) * G::BY + (b + G::NG)) * G::BX + (a + G::HX) - sp;
   const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX) - sm;
   T Phi[NV];
-  face_flux_rot<T>(sPc, sMc, sp, sm, d, par, Phi);
+  face_flux_rot<T, R>(sPc, sMc, sp, sm, d, par, Phi);
   T* o = sF + off + (c * e1 + b) * e0 + a;
   o[0] = Phi[0];
   o[4 * G::NF] = Phi[4];
@@ -387,14 +402,14 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
 
 // Source item: the geometric and cleaning sources (a6) of 32 cells -> sR[(q-1) * NC + cell], q = 1..8
 // (the D equation has no source).  Needs no flux, so it fills the scheduling gaps of the face items.
-template <typename T>
+template <typename T, int R>
 __device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, const T* sP, const T* sM, T* sR,
                                             int cell, int x0, int y0, int z0) {
-  using G = TileGeom<T>;
+  using G = TileGeom<T, R>;
   const int a = cell % G::TX, r = cell / G::TX;
   const int b = swz(r % G::TY), c = r / G::TY;
   if (x0 + a >= L.n[0] || y0 + b >= L.n[1] || z0 + c >= L.n[2]) return;
-  const T* sPc = sP + ((c + NG) * G::BY + (b + NG)) * G::BX + (a + G::HX);
+  const T* sPc = sP + ((c + G::NG) * G::BY + (b + G::NG)) * G::BX + (a + G::HX);
   const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX);
   T q[NV], m[NM];
 #pragma unroll
@@ -407,25 +422,25 @@ __device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, 
   const T idet = rcp_(det);
 #pragma unroll
   for (int a6 = 0; a6 < 6; a6++) gi[a6] = cf[a6] * idet;
-  T R[NV];
+  T Rs[NV];
 #pragma unroll
-  for (int v = 0; v < NV; v++) R[v] = 0;
-  add_sources_staged(L, sMc, m, q, par, gi, sq, R);
-  if (par.energy_var) R[4] = 0;  // R1b: no source on a fixed metric
+  for (int v = 0; v < NV; v++) Rs[v] = 0;
+  add_sources_staged<T, R>(L, sMc, m, q, par, gi, sq, Rs);
+  if (par.energy_var) Rs[4] = 0;  // R1b: no source on a fixed metric
 #pragma unroll
-  for (int v = 1; v < NV; v++) sR[(v - 1) * G::NC + cell] = R[v];
+  for (int v = 1; v < NV; v++) sR[(v - 1) * G::NC + cell] = Rs[v];
 }
 
 // One thread: the two TMA boxes of `tile` (primitives, metric), completion on `bar`.
-template <typename T>
+template <typename T, int R>
 __device__ __forceinline__ void issue_loads(const CUtensorMap* tmP, const CUtensorMap* tmM, const Layout& L, T* sP, T* sM,
                                             unsigned bar, int tile, int ntx, int nty) {
-  using G = TileGeom<T>;
+  using G = TileGeom<T, R>;
   const int tx = tile % ntx, r = tile / ntx;
   const int x0 = tx * G::TX, y0 = (r % nty) * G::TY, z0 = (r / nty) * G::TZ;
   mbar_expect_tx(bar, G::TX_BYTES);
   // storage coordinates of tile-local cell (-HX,-2,-2) / (-HX,-1,-1); out-of-range parts are zero-filled
-  tma_load_4d(smem_addr(sP), tmP, bar, x0 + L.ox - G::HX, y0 + L.g[1] - NG, z0 + L.g[2] - NG, 0);
+  tma_load_4d(smem_addr(sP), tmP, bar, x0 + L.ox - G::HX, y0 + L.g[1] - G::NG, z0 + L.g[2] - G::NG, 0);
   tma_load_4d(smem_addr(sM), tmM, bar, x0 + L.ox - G::HX, y0 + L.g[1] - 1, z0 + L.g[2] - 1, 0);
 }
 
@@ -437,13 +452,13 @@ __device__ __forceinline__ void issue_loads(const CUtensorMap* tmP, const CUtens
 // T2 is the arithmetic type of phase 2.  T2 = T: pure fp64 or pure fp32.  T = float with
 // T2 = double is the paper's mixed mode: storage, reconstruction and face fluxes in
 // fp32; flux difference, Runge-Kutta combine and the primitive recovery in fp64.
-template <typename T, typename T2>
-__global__ void __launch_bounds__(Tile<T>::NT, 1)
+template <typename T, typename T2, int R>
+__global__ void __launch_bounds__(Tile<T, R>::NT, 1)
 k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmM, Layout L, Par<T> par,
           Par<T2> par2, const T* __restrict__ Uin, const T* __restrict__ U0, T* __restrict__ Uout,
           T* __restrict__ Pout, int stage, T2 dt, unsigned long long* __restrict__ counters, int ntx, int nty,
           int ntiles) {
-  using G = TileGeom<T>;
+  using G = TileGeom<T, R>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sP = reinterpret_cast<T*>(smem_raw + G::OFF_P);  // sP[field][z][y][x], halo 2 (HX in x)
   T* sM = reinterpret_cast<T*>(smem_raw + G::OFF_M);  // sM[field][z][y][x], halo 1 (HX in x)
@@ -458,12 +473,12 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     *queue = 0;
   }
   __syncthreads();
-  if (threadIdx.x == 0 && (int)blockIdx.x < ntiles) issue_loads<T>(&tmP, &tmM, L, sP, sM, bar, blockIdx.x, ntx, nty);
+  if (threadIdx.x == 0 && (int)blockIdx.x < ntiles) issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, blockIdx.x, ntx, nty);
 
   // this thread's cell of phase 2 (one cell per thread), tile-local
   const int ca = threadIdx.x % G::TX, cr = threadIdx.x / G::TX;
   const int cb = swz(cr % G::TY), cc = cr / G::TY;
-  const T* sPc = sP + ((cc + NG) * G::BY + (cb + NG)) * G::BX + (ca + G::HX);
+  const T* sPc = sP + ((cc + G::NG) * G::BY + (cb + G::NG)) * G::BX + (ca + G::HX);
   const T* sMc = sM + ((cc + 1) * G::MY + (cb + 1)) * G::BX + (ca + G::HX);
   int fail = 0, reset = 0, pfl = 0, it = 0;
   unsigned parity = 0;
@@ -484,8 +499,8 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       if (lane == 0) t = atomicAdd(queue, 1);
       t = __shfl_sync(0xffffffffu, t, 0);
       if (t >= G::NFACE_TASKS + G::NSRC_TASKS) break;
-      if (t < G::NFACE_TASKS) face_task<T>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
-      else source_task<T>(L, par, sP, sM, sR, (t - G::NFACE_TASKS) * 32 + lane, x0, y0, z0);
+      if (t < G::NFACE_TASKS) face_task<T, R>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
+      else source_task<T, R>(L, par, sP, sM, sR, (t - G::NFACE_TASKS) * 32 + lane, x0, y0, z0);
     }
     // inputs of this thread's cell: conserved state from HBM (latency overlaps the barrier wait),
     // previous primitives and metric from the staged boxes (free for the next tile afterwards)
@@ -505,37 +520,37 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     __syncthreads();  // all fluxes and sources are in shared memory; nobody reads sP / sM any more
     if (threadIdx.x == 0) {
       *queue = 0;
-      if (tile + (int)gridDim.x < ntiles) issue_loads<T>(&tmP, &tmM, L, sP, sM, bar, tile + gridDim.x, ntx, nty);
+      if (tile + (int)gridDim.x < ntiles) issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, tile + gridDim.x, ntx, nty);
     }
 
     // ---- phase 2: one cell per thread, arithmetic in T2 ----
     // 2a: right-hand side from the fluxes and sources in shared memory; after the barrier below sF / sR are
     // free, so a warp that finishes 2b early goes straight on to the next tile's work queue (the Newton
     // iteration counts differ from cell to cell, and no barrier follows them).
-    T2 R[NV];
+    T2 Rh[NV];
     if (cell_ok) {
-      R[0] = 0;
+      Rh[0] = 0;
 #pragma unroll
-      for (int v = 1; v < NV; v++) R[v] = (T2)sR[(v - 1) * G::NC + threadIdx.x];
+      for (int v = 1; v < NV; v++) Rh[v] = (T2)sR[(v - 1) * G::NC + threadIdx.x];
       if (L.g[0]) {
         const T2 ih = par2.ih[0];
         const T* o = sF + (cc * G::TY + cb) * (G::TX + 1) + ca;
 #pragma unroll
-        for (int v = 0; v < NV; v++) R[v] -= ((T2)o[v * G::NF + 1] - (T2)o[v * G::NF]) * ih;
+        for (int v = 0; v < NV; v++) Rh[v] -= ((T2)o[v * G::NF + 1] - (T2)o[v * G::NF]) * ih;
       }
       if (L.g[1]) {
         const T2 ih = par2.ih[1];
         const T* o = sF + G::NFX + (cc * (G::TY + 1) + cb) * G::TX + ca;
 #pragma unroll
-        for (int v = 0; v < NV; v++) R[v] -= ((T2)o[v * G::NF + G::TX] - (T2)o[v * G::NF]) * ih;
+        for (int v = 0; v < NV; v++) Rh[v] -= ((T2)o[v * G::NF + G::TX] - (T2)o[v * G::NF]) * ih;
       }
       if (L.g[2]) {
         const T2 ih = par2.ih[2];
         const T* o = sF + G::NFX + G::NFY + (cc * G::TY + cb) * G::TX + ca;
 #pragma unroll
-        for (int v = 0; v < NV; v++) R[v] -= ((T2)o[v * G::NF + G::TX * G::TY] - (T2)o[v * G::NF]) * ih;
+        for (int v = 0; v < NV; v++) Rh[v] -= ((T2)o[v * G::NF + G::TX * G::TY] - (T2)o[v * G::NF]) * ih;
       }
-      if (!par2.cleaning) R[8] = 0;
+      if (!par2.cleaning) Rh[8] = 0;
     }
     __syncthreads();  // everybody has read sF / sR: the next tile's phase 1 may overwrite them
     if (cell_ok) {  // 2b
@@ -543,7 +558,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       T2 un[NV];
 #pragma unroll
       for (int v = 0; v < NV; v++) {
-        T2 u1 = (T2)u[v] + dt * R[v];
+        T2 u1 = (T2)u[v] + dt * Rh[v];
         if (stage == 1) u1 = T2(0.75) * (T2)u0[v] + T2(0.25) * u1;
         if (stage == 2) u1 = T2(1.0 / 3.0) * (T2)u0[v] + T2(2.0 / 3.0) * u1;
         un[v] = u1;
