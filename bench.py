@@ -199,6 +199,10 @@ def run_gpu(args):
     n, dtype = args.n, args.dtype
     K, W = args.steps, max(args.warmup, 3)
     w, wname = make_workload(wl, args.workload, n)
+    if args.recon == "ppm":
+        import dataclasses
+        w = dataclasses.replace(w, params={**w.params, "recon": 1})
+        wname += ", PPM reconstruction"
     stream = torch.cuda.current_stream()
     es = 8 if dtype == "f64" else 4
     shard = args.shard and world > 1
@@ -349,6 +353,8 @@ def main():
     ap.add_argument("--ref-n", type=int, default=128, help="sub-grid the CPU oracle is timed on")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--recon", default="mc", choices=["mc", "ppm"],
+                    help="reconstruction (PAPER.md:128): MC-limited linear (the metric's configuration) or PPM")
     ap.add_argument("--shard", action="store_true",
                     help="with --gpus N > 1: cut the one box into N z-slabs with a halo exchange per substep "
                          "(strong scaling) instead of N independent replicas (weak scaling, the default)")
