@@ -1,19 +1,22 @@
 // hz_substep.cuh -- one Runge-Kutta substep as ONE kernel (rows a1-a9 of DESIGN.md section 2).
 //
-// A block owns a tile of TX x TY x TZ cells.
-// Blocks are persistent (one per SM) and take tiles round-robin.
+// Blocks are persistent (one per SM) and take tiles of TX x TY x TZ cells round-robin.  Per tile:
 //   Stage-in : one thread issues two TMA box loads (cp.async.bulk.tensor.4d): the 9 primitives of the
-//              tile with a 2-cell halo and the 10 metric components with a 1-cell halo (2 in x, so
-//              both boxes share the x origin) land in shared memory; everyone waits on one mbarrier.
-//   Phase 1  : the warps walk the list of the tile's faces (all three directions, each face exactly
-//              once): MC reconstruction, face metric, left/right states, HLLE.  The
-//              flux Phi of every face goes to shared memory; no face value ever goes to HBM.
-//   Phase 2  : every cell takes the flux difference of its six faces from shared memory, adds the
-//              geometric sources, combines the Runge-Kutta stage, recovers the
-//              primitives by Newton-Raphson with the atmosphere floors, and writes U and
-//              P -- P also into the ghost cells that mirror this cell (O9), so no separate
-//              boundary kernel runs.  P is double-buffered: neighbours still read the old primitives
-//              while this block writes the new ones.
+//              tile with an NG-cell halo (2 for MC, 3 for PPM) and the 10 metric components with a 1-cell
+//              halo (16 bytes of halo along x in both, so every box row starts 16-byte aligned) land in
+//              shared memory; everyone waits on one mbarrier.  The loads of the NEXT tile are issued as
+//              soon as phase 1 is over and fly during phase 2.
+//   Phase 1  : a work queue in shared memory, one item per warp at a time.  Face items: 32 faces of one
+//              direction, every face of the tile exactly once -- reconstruction (MC or PPM), face metric,
+//              left/right states, HLLE; the flux Phi goes to shared memory, never to HBM.
+//              Source items: the geometric and cleaning sources of 32 cells; they need no
+//              flux and fill the gaps the face items leave.
+//   Phase 2  : one cell per thread: flux difference of its six faces + sources from shared memory, Runge-
+//              Kutta stage, Newton-Raphson recovery with the atmosphere floors,
+//              then U and P are written -- P also into the ghost cells that mirror this cell (DESIGN.md
+//              O9), so no boundary kernel runs.  P is double-buffered: neighbours still read the old
+//              primitives while this block writes the new ones.  In the mixed mode
+//              this phase runs in fp64 on fp32 data.
 //
 // The face flux is written ONCE, for a sweep along axis 0: a sweep along axis d reads the vector and
 // metric components cyclically rotated by d (and stores the momentum and field fluxes rotated back),
