@@ -575,3 +575,29 @@ def test_ppm_differs_from_mc_and_slabs_exchange_three_planes():
     assert np.array_equal(grp.get_primitives(), pb)
     assert grp.slabs[0].hz.halo_bytes(0) == 9 * 3 * (grp.slabs[0].hz.halo_bytes(1) // (10 * 3))
     a.close(); b.close(); grp.close()
+
+
+@pytest.mark.parametrize("name", ["kerr", "tov", "alfven_3d"])
+def test_all_options_together_parity(name):
+    """PPM + the two-unknown recovery + the paper's energy variable in one run (the options are independent
+    switches in hz_params; this guards their combination), fp64 bar after a full RK3 step, and the mixed mode
+    at the fp32 bar after one substep."""
+    w = SMALL[name]()
+    wo = dataclasses.replace(w, params={**w.params, "recon": 1, "c2p_scheme": 1, "energy_var": 1})
+    o = oracle_for(wo)
+    hz = horizon(wo, "f64")
+    o.substeps(w.dt, 1)
+    ref1 = o.get_primitives()
+    o.substeps(w.dt, 2)
+    hz.substeps(w.dt, 3)
+    assert_parity(hz.get_primitives(), o.get_primitives(), TOL64_SUB, f"{name} all options")
+    Uo, Ug = o.get_conserved(), hz.get_conserved()
+    assert np.abs(Ug[4] - Uo[4]).sum() <= TOL64_SUB * np.abs(Uo[4]).sum()
+    hz.close()
+    hm = horizon(wo, "f32h")
+    hm.substeps(w.dt, 1)
+    got = hm.get_primitives()
+    flips = floor_flip_mask(got, ref1, w.params["rho_atm"], w.params["atm_tol"])
+    assert flips.sum() <= 2e-4 * w.ncell
+    assert_parity(got, ref1, TOL32_SUB, f"{name} all options mixed", mask=flips)
+    hm.close()
