@@ -299,43 +299,36 @@ __device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __r
 }
 
 // ---- a9 fused: store the primitives of cell (i,j,k) and of every ghost cell that mirrors it --------
+// Ghost images of interior coordinate c along axis d (O9): periodic -- c + n if c < ng, c - n if
+// c >= n - ng; zero gradient -- the edge cell fills the ng layers beyond it; external sides get none.
+__device__ __forceinline__ int image_count(const Layout& L, int d, int c) {
+  if (L.g[d] == 0) return 0;
+  const int n = L.n[d];
+  if (L.bc[d] == 0) return (c < L.ng) + (c >= n - L.ng);
+  if (c == 0 && bc_side(L.bc[d], 0) == 1) return L.ng;
+  if (c == n - 1 && bc_side(L.bc[d], 1) == 1) return L.ng;
+  return 0;
+}
+// t = 0 is the cell itself, t = 1 .. image_count its images
+__device__ __forceinline__ int image_coord(const Layout& L, int d, int c, int t) {
+  if (t == 0) return c;
+  const int n = L.n[d];
+  if (L.bc[d] == 0) return (t == 1 && c < L.ng) ? c + n : c - n;
+  return c == 0 ? -t : n - 1 + t;
+}
 template <typename T>
 __device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __restrict__ Pout, int i, int j, int k,
                                                         const T* q) {
-  const int c3[3] = {i, j, k};
-  int dst[3][4], cnt[3];   // the cell itself and up to 3 images per axis
-  bool plain = true;
+  const long long id0 = L.idx(i, j, k);
 #pragma unroll
-  for (int d = 0; d < 3; d++) {
-    const int c = c3[d], n = L.n[d];
-    dst[d][0] = c;
-    cnt[d] = 1;
-    if (L.g[d]) {
-      if (L.bc[d] == 0) {  // periodic wrap
-        if (c < L.ng) dst[d][cnt[d]++] = c + n;
-        if (c >= n - L.ng) dst[d][cnt[d]++] = c - n;
-      } else {             // zero gradient: the edge cell fills its ghost layers; external sides are left alone
-        if (c == 0 && bc_side(L.bc[d], 0) == 1) {
-          for (int t = 1; t <= L.ng; t++) dst[d][t] = -t;
-          cnt[d] = 1 + L.ng;
-        } else if (c == n - 1 && bc_side(L.bc[d], 1) == 1) {
-          for (int t = 1; t <= L.ng; t++) dst[d][t] = n - 1 + t;
-          cnt[d] = 1 + L.ng;
-        }
-      }
-    }
-    plain = plain && cnt[d] == 1;
-  }
-  if (plain) {
-    const long long id = L.idx(i, j, k);
-#pragma unroll
-    for (int v = 0; v < NV; v++) Pout[v * L.fs + id] = q[v];
-    return;
-  }
-  for (int c = 0; c < cnt[2]; c++)
-    for (int b = 0; b < cnt[1]; b++)
-      for (int a = 0; a < cnt[0]; a++) {
-        const long long id = L.idx(dst[0][a], dst[1][b], dst[2][c]);
+  for (int v = 0; v < NV; v++) Pout[v * L.fs + id0] = q[v];
+  const int ci = image_count(L, 0, i), cj = image_count(L, 1, j), ck = image_count(L, 2, k);
+  if ((ci | cj | ck) == 0) return;   // not within reach of a boundary: the common case
+  for (int c = 0; c <= ck; c++)
+    for (int b = 0; b <= cj; b++)
+      for (int a = 0; a <= ci; a++) {
+        if ((a | b | c) == 0) continue;
+        const long long id = L.idx(image_coord(L, 0, i, a), image_coord(L, 1, j, b), image_coord(L, 2, k, c));
 #pragma unroll
         for (int v = 0; v < NV; v++) Pout[v * L.fs + id] = q[v];
       }
@@ -496,12 +489,15 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     mbar_wait(bar, parity);
 
     // ---- phase 1: work queue of face items, then source items ----
+    // The next item number is fetched (one shared-memory atomic by lane 0) BEFORE the current item is
+    // worked on and broadcast only when it is needed, so the atomic's latency hides behind the item.
+    int fetched = 0;
+    if (lane == 0) fetched = atomicAdd(queue, 1);
 #pragma unroll 1
     for (;;) {
-      int t = 0;
-      if (lane == 0) t = atomicAdd(queue, 1);
-      t = __shfl_sync(0xffffffffu, t, 0);
+      const int t = __shfl_sync(0xffffffffu, fetched, 0);
       if (t >= G::NFACE_TASKS + G::NSRC_TASKS) break;
+      if (lane == 0) fetched = atomicAdd(queue, 1);
       if (t < G::NFACE_TASKS) face_task<T, R>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
       else source_task<T, R>(L, par, sP, sM, sR, (t - G::NFACE_TASKS) * 32 + lane, x0, y0, z0);
     }
