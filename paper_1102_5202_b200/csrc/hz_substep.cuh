@@ -365,7 +365,8 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
   asm volatile("" : "+r"(d));
   const int off = d == 0 ? 0 : (d == 1 ? G::NFX : G::NFX + G::NFY);                 // first face of d in sF
   const int f = (task - (d == 0 ? 0 : (d == 1 ? G::WX : G::WX + G::WY))) * 32 + lane;  // face number within d
-  if (L.g[d] == 0) return;
+  // (no L.g[d]: indexing a kernel parameter with a run-time d makes the compiler copy it to local memory)
+  if ((d == 0 ? L.g[0] : (d == 1 ? L.g[1] : L.g[2])) == 0) return;
   if (f >= (d == 0 ? G::NFX : (d == 1 ? G::NFY : G::NFZ))) return;                     // partly empty last item
   // face coordinates inside the tile: f = (c * e1 + b) * e0 + a with e0 = TX (+1 for x faces),
   // e1 = TY (+1 for y faces); the quotients by multiply-shift (d is a run-time value here)
