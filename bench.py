@@ -40,7 +40,7 @@ ALGO_FLOPS = {"f64": 3700.0, "f32": 2900.0, "f32h": 2900.0}
 SMS, LANES = 148, {"f64": 64, "f32": 128, "f32h": 128}
 # ncu dram__bytes_read.sum + dram__bytes_write.sum of one k_substep launch at 128^3, per zone
 # (profiles/r01_substep.md); scaled to the launch's zones below
-TRAFFIC_BYTES_PER_ZONE = {"f64": 497.0, "f32": 268.0, "f32h": 268.0}
+TRAFFIC_BYTES_PER_ZONE = {"f64": 494.0, "f32": 263.0, "f32h": 263.0}
 
 
 def peaks():
