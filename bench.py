@@ -294,6 +294,8 @@ def run_gpu(args):
     alu_peak = SMS * LANES[dtype] * 2 * sm_max * 1e6 / 1e12      # TFLOP/s
     achieved = flops_per_launch / avg_s / 1e12
     hbm_achieved = bytes_per_launch / avg_s / 1e9
+    from paper_1102_5202_b200.binding import fma_peak
+    measured_alu = fma_peak("f64" if dtype == "f64" else "f32")   # FMA-chain microbenchmark, after the timed region
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
                 "frac": achieved / alu_peak,
                 "traffic": TRAFFIC_BYTES_PER_ZONE[dtype] * ncell,
@@ -301,6 +303,7 @@ def run_gpu(args):
                 "algorithmic_flops_per_launch": flops_per_launch, "algorithmic_bytes_per_launch": bytes_per_launch,
                 "avg_launch_ms": avg_s * 1e3, "share_of_step": dom_ms / tot_ms if tot_ms > 0 else None,
                 "kernels_ms_per_substep": {k: v[0] / (K * SUBSTEPS_PER_STEP) for k, v in prof.items() if v[1]},
+                "alu_peak_measured": measured_alu, "frac_of_measured_alu_peak": achieved / measured_alu,
                 "hbm_achieved_gbs": hbm_achieved, "hbm_peak_gbs": hbm_gbs, "hbm_frac": hbm_achieved / hbm_gbs,
                 "hbm_peak_source": peak_src,
                 "traffic_source": "ncu dram bytes of one launch at 128^3, per zone (profiles/r01_substep.md)"}

@@ -159,6 +159,12 @@ int hz_halo_unpack(hz_ctx* ctx, int which, int side, const void* device_buf);
 /* Number of kernels this context has launched since hz_create (bench.py's gpu_launches). */
 long long hz_launch_count(const hz_ctx* ctx);
 
+/* Measured throughput of the plain FMA pipe in `dtype` (HZ_F32 or HZ_F64), TFLOP/s with FMA = 2 flops:
+ * a kernel of nothing but independent FMAs on every SM, best of three timed launches on the default stream.
+ * It is the measured counterpart of the derived ALU peak the roofline is quoted against.
+ * Needs no context.  HZ_ECUDA without a device. */
+int hz_fma_peak(int dtype, double* tflops);
+
 /* Per-kernel device timing of the substep kernels, for the roofline report (PAPER.md:190-194 times
  * the main loop only).  hz_profile(ctx, 1) brackets every later substep kernel launch with CUDA
  * events on the context stream; hz_profile_read synchronises, adds up the elapsed milliseconds and

@@ -13,7 +13,7 @@ HZ_OK, HZ_EINVAL, HZ_ENOMEM, HZ_ECUDA, HZ_ESTATE = 0, -1, -2, -3, -4
 # every symbol include/hz.h declares (tests check the library exports each of them)
 SYMBOLS = ["hz_default_params", "hz_state_bytes", "hz_create", "hz_destroy", "hz_set_stream", "hz_set_metric",
            "hz_set_primitives", "hz_step", "hz_substeps", "hz_get_primitives", "hz_get_psi", "hz_get_conserved",
-           "hz_diagnostics", "hz_halo_bytes", "hz_halo_pack", "hz_halo_unpack", "hz_launch_count", "hz_profile", "hz_profile_read", "hz_kernel_name",
+           "hz_diagnostics", "hz_halo_bytes", "hz_halo_pack", "hz_halo_unpack", "hz_launch_count", "hz_fma_peak", "hz_profile", "hz_profile_read", "hz_kernel_name",
            "hz_strerror"]
 HZ_NKERNELS = 4
 
@@ -93,6 +93,7 @@ def lib():
         L.hz_halo_bytes.argtypes = [vp, ip, C.POINTER(C.c_size_t)]
         L.hz_halo_pack.argtypes = [vp, ip, ip, vp]
         L.hz_halo_unpack.argtypes = [vp, ip, ip, vp]
+        L.hz_fma_peak.argtypes = [ip, C.POINTER(C.c_double)]
         L.hz_launch_count.argtypes = [vp]
         L.hz_launch_count.restype = C.c_longlong
         L.hz_profile.argtypes = [vp, ip]
@@ -115,6 +116,13 @@ def _ptr(a):
     if isinstance(a, np.ndarray):
         return C.c_void_p(a.ctypes.data)
     return C.c_void_p(a.data_ptr())  # torch.Tensor
+
+
+def fma_peak(dtype="f64"):
+    """Measured FMA-pipe throughput in TFLOP/s (hz_fma_peak)."""
+    t = C.c_double(0)
+    _chk(lib().hz_fma_peak(HZ_F64 if dtype == "f64" else HZ_F32, C.byref(t)), "hz_fma_peak")
+    return t.value
 
 
 class Horizon:

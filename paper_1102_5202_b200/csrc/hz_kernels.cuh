@@ -67,6 +67,23 @@ __global__ void k_halo_copy(Layout L, T* __restrict__ F, int nf, int k0, T* __re
   }
 }
 
+// ---- hz_fma_peak: what the plain FMA pipe sustains (the denominator of the ALU roofline) ----
+// 16 independent accumulators per thread, `iters` trips of 16 FMAs each; nothing but FMAs in the loop.
+template <typename T>
+__global__ void __launch_bounds__(256) k_fma_peak(T* __restrict__ out, int iters, T a, T b) {
+  T acc[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) acc[i] = (T)(threadIdx.x + i);
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 16; i++) acc[i] = acc[i] * a + b;
+  }
+  T s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += acc[i];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 // ---- hz_set_metric: interior-only planes -> padded SoA, with validation -------------------------
 template <typename T>
 __global__ void k_pack_metric(Layout L, const T* __restrict__ alpha, const T* __restrict__ beta3,

@@ -566,6 +566,36 @@ int hz_halo_unpack(hz_ctx* c, int which, int side, const void* device_buf) {
 
 long long hz_launch_count(const hz_ctx* c) { return c ? c->launches : 0; }
 
+int hz_fma_peak(int dtype, double* tflops) {
+  if (!tflops || (dtype != HZ_F32 && dtype != HZ_F64)) return HZ_EINVAL;
+  int ndev = 0, nsm = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return HZ_ECUDA; }
+  int dev = 0;
+  cudaGetDevice(&dev);
+  HZ_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+  const int blocks = nsm * 8, threads = 256, iters = 1 << 14;
+  void* buf = nullptr;
+  HZ_CUDA(cudaMalloc(&buf, (size_t)blocks * threads * 8));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; rep++) {   // first launch warms up; best of the rest
+    cudaEventRecord(e0, 0);
+    if (dtype == HZ_F64) k_fma_peak<double><<<blocks, threads>>>((double*)buf, iters, 1.0000001, 1e-9);
+    else k_fma_peak<float><<<blocks, threads>>>((float*)buf, iters, 1.0000001f, 1e-9f);
+    cudaEventRecord(e1, 0);
+    cudaEventSynchronize(e1);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(buf);
+  if (cudaGetLastError() != cudaSuccess) return HZ_ECUDA;
+  *tflops = 2.0 * 16.0 * iters * (double)blocks * threads / (best * 1e-3) / 1e12;
+  return HZ_OK;
+}
+
 int hz_profile(hz_ctx* c, int enable) {
   if (!c) return HZ_EINVAL;
   HZ_CUDA(cudaStreamSynchronize(c->stream));
