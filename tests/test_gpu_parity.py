@@ -601,3 +601,13 @@ def test_all_options_together_parity(name):
     assert flips.sum() <= 2e-4 * w.ncell
     assert_parity(got, ref1, TOL32_SUB, f"{name} all options mixed", mask=flips)
     hm.close()
+
+
+def test_fma_peak_is_plausible():
+    """hz_fma_peak: the measured FMA-pipe throughput the ALU roofline is compared with.  fp32 issues at twice
+    the fp64 rate on this part; both must be positive and below the derived unit-count peak."""
+    from paper_1102_5202_b200.binding import fma_peak
+    f64, f32 = fma_peak("f64"), fma_peak("f32")
+    assert 1.0 < f64 < 148 * 64 * 2 * 2.1e9 / 1e12 * 1.02
+    assert 1.0 < f32 < 148 * 128 * 2 * 2.1e9 / 1e12 * 1.02
+    assert 1.5 < f32 / f64 < 2.5
