@@ -67,6 +67,40 @@ __global__ void k_halo_copy(Layout L, T* __restrict__ F, int nf, int k0, T* __re
   }
 }
 
+// ---- static coefficients of the cleaning sources (O6 / R14) -----------------------------------
+// cln[k] = sum_j d_j(alpha sqrt(gamma) gamma^{kj}), k = x y z;  cln[3] = sum_j d_j(sqrt(gamma) beta^j), centred
+// differences of the stored metric at interior cells.  The metric is fixed, so this runs once per
+// hz_set_metric (and again when ghost planes of the metric arrive through hz_halo_unpack).
+template <typename T>
+__global__ void k_clean_static(Layout L, const T* __restrict__ met, T* __restrict__ cln) {
+  const long long n = L.ncell();
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  int i, j, k;
+  cell_of(L, t, i, j, k);
+  const long long id = L.idx(i, j, k);
+  T dQ[3] = {0, 0, 0}, dRb = 0;
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    if (L.g[d] == 0) continue;
+    const long long s = L.stride(d);
+    const T i2h = T(0.5) * (T)(1.0 / L.h[d]);
+    T mp[NM], mm[NM];
+    load_fields(met, L.fs, id + s, NM, mp);
+    load_fields(met, L.fs, id - s, NM, mm);
+    T cp[6], cm[6];
+    const T dp = cofactors(mp + GXX, cp), dn = cofactors(mm + GXX, cm);
+    const T sp = sqrt_(dp), sn = sqrt_(dn);
+    const T ap = div_(mp[AL], sp), am = div_(mm[AL], sn);  // alpha sqrt(gamma) gamma^{kd} = alpha cof_kd / sqrt(gamma)
+#pragma unroll
+    for (int kk = 0; kk < 3; kk++) dQ[kk] += (ap * cp[sym(kk, d)] - am * cm[sym(kk, d)]) * i2h;
+    dRb += (sp * mp[BEX + d] - sn * mm[BEX + d]) * i2h;
+  }
+#pragma unroll
+  for (int kk = 0; kk < 3; kk++) cln[kk * L.fs + id] = dQ[kk];
+  cln[3 * L.fs + id] = dRb;
+}
+
 // ---- hz_fma_peak: what the plain FMA pipe sustains (the denominator of the ALU roofline) ----
 // 16 independent accumulators per thread, `iters` trips of 16 FMAs each; nothing but FMAs in the loop.
 template <typename T>

@@ -54,7 +54,7 @@ Layout make_layout(const hz_grid& G, int dtype, int ng) {
 
 // Memory plan: offsets (bytes) of every resident array inside the one device buffer.
 struct Plan {
-  size_t met, P[2], U[2], staging, partials, diag_out, counters, err, total;
+  size_t met, cln, P[2], U[2], staging, partials, diag_out, counters, err, total;
   int diag_blocks;
 };
 Plan make_plan(const Layout& L, int dtype) {
@@ -64,6 +64,7 @@ Plan make_plan(const Layout& L, int dtype) {
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 256); return r; };
   p.met = take(NM * field);
+  p.cln = take(4 * field);   // static coefficients of the cleaning sources (k_clean_static)
   p.P[0] = take(NV * field);
   p.P[1] = take(NV * field);
   p.U[0] = take(NV * field);
@@ -112,6 +113,7 @@ struct hz_ctx {
   std::vector<int> ev_kind;           // kind of each recorded pair
 
   template <typename T> T* met() const { return (T*)(base + plan.met); }
+  template <typename T> T* cln() const { return (T*)(base + plan.cln); }
   template <typename T> T* P(int w) const { return (T*)(base + plan.P[w]); }
   template <typename T> T* U(int w) const { return (T*)(base + plan.U[w]); }
   template <typename T> T* staging() const { return (T*)(base + plan.staging); }
@@ -203,6 +205,8 @@ int set_metric_t(hz_ctx* c, const void* alpha, const void* beta3, const void* ga
   const long long ntot = (long long)L.N[0] * L.N[1] * L.N[2];
   k_fill_ghosts<T><<<nblocks(ntot, 256), 256, 0, c->stream>>>(L, c->met<T>(), NM);
   HZ_LAUNCHED(c);
+  k_clean_static<T><<<nblocks(n, 256), 256, 0, c->stream>>>(L, c->met<T>(), c->cln<T>());
+  HZ_LAUNCHED(c);
   int flag = 0;
   if ((rc = read_err(c, &flag))) return rc;
   c->have_prim = false;
@@ -259,10 +263,11 @@ int substep_tr(hz_ctx* c, double dt) {
     ProfScope ps(c, K_SUBSTEP);
     if (sizeof(T) == 4 && c->dtype == HZ_F32_F64)  // fp32 storage and faces, fp64 flux difference / RK / con2prim
       k_substep<float, double, R><<<grid, G::NT, G::SMEM, c->stream>>>(
-          c->tmP[c->pcur], c->tmM, L, make_par<float>(c), make_par<double>(c), (const float*)Uin, (const float*)U0,
+          c->tmP[c->pcur], c->tmM, L, make_par<float>(c), make_par<double>(c), (const float*)c->cln<T>(),
+          (const float*)Uin, (const float*)U0,
           (float*)Uout, (float*)c->P<T>(1 - c->pcur), st, dt, c->counters(), ntx, nty, (int)ntiles);
     else
-      k_substep<T, T, R><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, par, Uin, U0, Uout,
+      k_substep<T, T, R><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, par, c->cln<T>(), Uin, U0, Uout,
                                                             c->P<T>(1 - c->pcur), st, (T)dt, c->counters(), ntx, nty,
                                                             (int)ntiles);
   }
@@ -393,6 +398,10 @@ int halo_copy_t(hz_ctx* c, int which, int k0, void* buf, int unpack) {
   const unsigned nb = (unsigned)((tot + 255) / 256 < 4736 ? (tot + 255) / 256 : 4736);
   k_halo_copy<T><<<nb, 256, 0, c->stream>>>(c->L, F, nf, k0, (T*)buf, unpack);
   HZ_LAUNCHED(c);
+  if (unpack && which == HZ_HALO_METRIC) {  // new ghost planes of the metric: its static derivatives follow
+    k_clean_static<T><<<nblocks(c->L.ncell(), 256), 256, 0, c->stream>>>(c->L, c->met<T>(), c->cln<T>());
+    HZ_LAUNCHED(c);
+  }
   return HZ_OK;
 }
 

@@ -255,11 +255,11 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
 // sMc: staged metric at the cell (field 0).  Same arithmetic as add_sources (hz_kernels.cuh).
 template <typename T, int R>
 __device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __restrict__ sMc, const T* m, const T* q,
-                                                   const Par<T>& par, const T* gi, T sq, T* Rs) {
+                                                   const Par<T>& par, const T* gi, T sq, const T* cl4, T* Rs) {
   using G = TileGeom<T, R>;
   T dm[3][NM];
-  T dQ[3] = {0, 0, 0};  // sum_j d_j(alpha sqrt(gamma) gamma^{kj})
-  T dRb = 0;            // sum_j d_j(sqrt(gamma) beta^j)
+  // cl4 = (sum_j d_j(alpha sqrt(gamma) gamma^{kj}), k = x y z; sum_j d_j(sqrt(gamma) beta^j)): the metric does
+  // not change in time, so these four coefficients of the cleaning sources are computed once (k_clean_static)
 #pragma unroll
   for (int d = 0; d < 3; d++) {
     if (L.g[d] == 0) {
@@ -274,25 +274,16 @@ __device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __r
     for (int a = 0; a < NM; a++) { mp[a] = sMc[a * G::MFS + s]; mm[a] = sMc[a * G::MFS - s]; }
 #pragma unroll
     for (int a = 0; a < NM; a++) dm[d][a] = (mp[a] - mm[a]) * i2h;
-    if (par.cleaning) {
-      T cp[6], cm[6];
-      const T dp = cofactors(mp + GXX, cp), dn = cofactors(mm + GXX, cm);
-      const T sp = sqrt_(dp), sn = sqrt_(dn);
-      const T ap = div_(mp[AL], sp), am = div_(mm[AL], sn);  // alpha sqrt(gamma) gamma^{kd} = alpha cof_kd / sqrt(gamma)
-#pragma unroll
-      for (int k = 0; k < 3; k++) dQ[k] += (ap * cp[sym(k, d)] - am * cm[sym(k, d)]) * i2h;
-      dRb += (sp * mp[BEX + d] - sn * mm[BEX + d]) * i2h;
-    }
   }
   fluid_source(q, m, dm, par, gi, sq, Rs);
   if (par.cleaning) {  // cleaning sources (R14), not multiplied by alpha
 #pragma unroll
     for (int k = 0; k < 3; k++) {
       const T adv = q[BX] * dm[0][BEX + k] + q[BY] * dm[1][BEX + k] + q[BZ] * dm[2][BEX + k];
-      Rs[5 + k] += -sq * adv + q[PSI] * dQ[k];
+      Rs[5 + k] += -sq * adv + q[PSI] * cl4[k];
     }
     const T Bda = q[BX] * dm[0][AL] + q[BY] * dm[1][AL] + q[BZ] * dm[2][AL];
-    Rs[8] += sq * Bda - q[PSI] * dRb - m[AL] * par.kappa * sq * q[PSI];
+    Rs[8] += sq * Bda - q[PSI] * cl4[3] - m[AL] * par.kappa * sq * q[PSI];
   } else {
     Rs[8] = 0;
   }
@@ -401,7 +392,7 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
 // (the D equation has no source).  Needs no flux, so it fills the scheduling gaps of the face items.
 template <typename T, int R>
 __device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, const T* sP, const T* sM, T* sR,
-                                            int cell, int x0, int y0, int z0) {
+                                            const T* __restrict__ cln, int cell, int x0, int y0, int z0) {
   using G = TileGeom<T, R>;
   const int a = cell % G::TX, r = cell / G::TX;
   const int b = swz(r % G::TY), c = r / G::TY;
@@ -422,7 +413,13 @@ __device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, 
   T Rs[NV];
 #pragma unroll
   for (int v = 0; v < NV; v++) Rs[v] = 0;
-  add_sources_staged<T, R>(L, sMc, m, q, par, gi, sq, Rs);
+  T cl4[4] = {0, 0, 0, 0};
+  if (par.cleaning) {
+    const long long id = L.idx(x0 + a, y0 + b, z0 + c);
+#pragma unroll
+    for (int v = 0; v < 4; v++) cl4[v] = cln[v * L.fs + id];
+  }
+  add_sources_staged<T, R>(L, sMc, m, q, par, gi, sq, cl4, Rs);
   if (par.energy_var) Rs[4] = 0;  // R1b: no source on a fixed metric
 #pragma unroll
   for (int v = 1; v < NV; v++) sR[(v - 1) * G::NC + cell] = Rs[v];
@@ -452,7 +449,8 @@ __device__ __forceinline__ void issue_loads(const CUtensorMap* tmP, const CUtens
 template <typename T, typename T2, int R>
 __global__ void __launch_bounds__(Tile<T, R>::NT, 1)
 k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmM, Layout L, Par<T> par,
-          Par<T2> par2, const T* __restrict__ Uin, const T* __restrict__ U0, T* __restrict__ Uout,
+          Par<T2> par2, const T* __restrict__ cln, const T* __restrict__ Uin, const T* __restrict__ U0,
+          T* __restrict__ Uout,
           T* __restrict__ Pout, int stage, T2 dt, unsigned long long* __restrict__ counters, int ntx, int nty,
           int ntiles) {
   using G = TileGeom<T, R>;
@@ -500,7 +498,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       if (t >= G::NFACE_TASKS + G::NSRC_TASKS) break;
       if (lane == 0) fetched = atomicAdd(queue, 1);
       if (t < G::NFACE_TASKS) face_task<T, R>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
-      else source_task<T, R>(L, par, sP, sM, sR, (t - G::NFACE_TASKS) * 32 + lane, x0, y0, z0);
+      else source_task<T, R>(L, par, sP, sM, sR, cln, (t - G::NFACE_TASKS) * 32 + lane, x0, y0, z0);
     }
     // inputs of this thread's cell: conserved state from HBM (latency overlaps the barrier wait),
     // previous primitives and metric from the staged boxes (free for the next tile afterwards)
