@@ -84,9 +84,40 @@ __device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
 __device__ __forceinline__ bool finite_(double x) { return isfinite(x); }
 __device__ __forceinline__ bool finite_(float x) { return isfinite(x); }
 
+// ---- two fp32 values in one register pair: the left and the right state of a face together ------------
+// Blackwell issues packed fp32 arithmetic (PTX add/mul/fma.f32x2, SASS FADD2 / FMUL2 / FFMA2) at the flop rate of
+// the scalar forms but in half the issue slots, and the fp32 kernel is bound by issue slots (profiles/
+// r01_substep.md).  The two states of a face run the same code on different data, so the fp32 face item
+// evaluates them as one F2 stream.  Transcendentals, min/max and selects stay per component.
+struct F2 {
+  float2 v;
+  __device__ __forceinline__ F2() {}
+  __device__ __forceinline__ F2(float a) { v = make_float2(a, a); }
+  __device__ __forceinline__ F2(float a, float b) { v = make_float2(a, b); }
+};
+__device__ __forceinline__ F2 mk2(float2 x) { F2 r; r.v = x; return r; }
+__device__ __forceinline__ F2 operator+(F2 a, F2 b) { return mk2(__fadd2_rn(a.v, b.v)); }
+__device__ __forceinline__ F2 operator-(F2 a, F2 b) { return mk2(__fadd2_rn(a.v, make_float2(-b.v.x, -b.v.y))); }
+__device__ __forceinline__ F2 operator*(F2 a, F2 b) { return mk2(__fmul2_rn(a.v, b.v)); }
+__device__ __forceinline__ F2 operator-(F2 a) { return F2(-a.v.x, -a.v.y); }
+__device__ __forceinline__ F2 operator+(float a, F2 b) { return F2(a) + b; }
+__device__ __forceinline__ F2 operator+(F2 a, float b) { return a + F2(b); }
+__device__ __forceinline__ F2 operator-(float a, F2 b) { return F2(a) - b; }
+__device__ __forceinline__ F2 operator-(F2 a, float b) { return a - F2(b); }
+__device__ __forceinline__ F2 operator*(float a, F2 b) { return F2(a) * b; }
+__device__ __forceinline__ F2 operator*(F2 a, float b) { return a * F2(b); }
+__device__ __forceinline__ F2& operator+=(F2& a, F2 b) { a = a + b; return a; }
+__device__ __forceinline__ F2 rsqrt_(F2 a) { return F2(rsqrt_(a.v.x), rsqrt_(a.v.y)); }
+__device__ __forceinline__ F2 sqrt_(F2 a) { return F2(sqrt_(a.v.x), sqrt_(a.v.y)); }
+__device__ __forceinline__ F2 rcp_(F2 a) { return F2(rcp_(a.v.x), rcp_(a.v.y)); }
+__device__ __forceinline__ F2 div_(F2 a, F2 b) { return a * rcp_(b); }
+__device__ __forceinline__ F2 div_(float a, F2 b) { return F2(a) * rcp_(b); }
+__device__ __forceinline__ F2 min_(F2 a, F2 b) { return F2(fminf(a.v.x, b.v.x), fminf(a.v.y, b.v.y)); }
+__device__ __forceinline__ F2 max_(F2 a, F2 b) { return F2(fmaxf(a.v.x, b.v.x), fmaxf(a.v.y, b.v.y)); }
+
 // Lower an index with the symmetric 3-metric stored as g6 = (xx, xy, xz, yy, yz, zz).
-template <typename T>
-__device__ __forceinline__ void lower(const T* g6, const T* a, T* l) {
+template <typename S, typename T>
+__device__ __forceinline__ void lower(const S* g6, const T* a, T* l) {
   l[0] = g6[0] * a[0] + g6[1] * a[1] + g6[2] * a[2];
   l[1] = g6[1] * a[0] + g6[3] * a[1] + g6[4] * a[2];
   l[2] = g6[2] * a[0] + g6[4] * a[1] + g6[5] * a[2];
@@ -193,8 +224,8 @@ __device__ __forceinline__ void ppm_face(T qm2, T qm1, T q0, T q1, T q2, T q3, T
 // -sqrt(-g) T^t_t = sqrt(gamma) [alpha (tau + D) - beta^j S_j]; source-free on a fixed metric.  The two maps
 // swap slot 4 of an undensitised (D, S_j, tau, ...) vector -- or, the map being linear, of a coordinate-flux
 // vector -- between tau and that variable on the metric m.
-template <typename T>
-__device__ __forceinline__ T tau_to_energy(const T* u, const T* m) {
+template <typename T, typename S>
+__device__ __forceinline__ T tau_to_energy(const T* u, const S* m) {
   return m[AL] * (u[4] + u[0]) - (m[BEX] * u[1] + m[BEY] * u[2] + m[BEZ] * u[3]);
 }
 template <typename T>

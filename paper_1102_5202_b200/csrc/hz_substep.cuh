@@ -108,10 +108,12 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map
 // ---- O1-O3 for one state in the frame of the sweep (axis 0 = sweep axis) ---------------------------
 // q = (rho, ut^0..2, p, B^0..2, psi), m = (alpha, beta^0..2, g00 g01 g02 g11 g12 g22), gi0[k] = gamma^{k0}.
 // U: undensitised conserved; F: coordinate flux along axis 0; lm, lp: coordinate signal speeds.
-template <typename T>
-__device__ __forceinline__ void state_flux0(const T* q, const T* m, const T* gi0, const Par<T>& par,
+// T is the value type (double, float, or F2 = the left and the right state as one packed fp32 stream),
+// S the scalar type of the face metric and the parameters, which both states share.
+template <typename T, typename S>
+__device__ __forceinline__ void state_flux0(const T* q, const S* m, const S* gi0, const Par<S>& par,
                                             T* U, T* F, T& lm, T& lp) {
-  const T* g = m + GXX;
+  const S* g = m + GXX;
   T utl[3], Bl[3];
   lower(g, q + UX, utl);
   lower(g, q + BX, Bl);
@@ -129,7 +131,7 @@ __device__ __forceinline__ void state_flux0(const T* q, const T* m, const T* gi0
   const T Z = rhoh * W2;
   const T D = q[RHO] * W;
   const T ZB = Z + B2;
-  const T al = m[AL], be = m[BEX];
+  const S al = m[AL], be = m[BEX];
   const T v0 = q[UX] * iW;
   const T vt = al * v0 - be;
   const T B0 = q[BX];
@@ -229,8 +231,18 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
   qL[RHO] = max_(qL[RHO], par.rho_atm); qL[PR] = max_(qL[PR], par.p_atm);
   qR[RHO] = max_(qR[RHO], par.rho_atm); qR[PR] = max_(qR[PR], par.p_atm);
   T UL[NV], FL[NV], UR[NV], FR[NV], lmL, lpL, lmR, lpR;
-  state_flux0(qL, mf, gi0, par, UL, FL, lmL, lpL);
-  state_flux0(qR, mf, gi0, par, UR, FR, lmR, lpR);
+  if constexpr (sizeof(T) == 4) {  // fp32: both states as one packed stream (F2, hz_physics.cuh)
+    F2 q2[NV], U2[NV], Fx2[NV], lm2, lp2;
+#pragma unroll
+    for (int v = 0; v < NV; v++) q2[v] = F2(qL[v], qR[v]);
+    state_flux0(q2, mf, gi0, par, U2, Fx2, lm2, lp2);
+#pragma unroll
+    for (int v = 0; v < NV; v++) { UL[v] = U2[v].v.x; UR[v] = U2[v].v.y; FL[v] = Fx2[v].v.x; FR[v] = Fx2[v].v.y; }
+    lmL = lm2.v.x; lmR = lm2.v.y; lpL = lp2.v.x; lpR = lp2.v.y;
+  } else {
+    state_flux0(qL, mf, gi0, par, UL, FL, lmL, lpL);
+    state_flux0(qR, mf, gi0, par, UR, FR, lmR, lpR);
+  }
   T lp = max_(lpL, lpR), lm = min_(lmL, lmR);
   if (par.cleaning) {  // light cone of the (B^d, psi) subsystem (O3)
     const T c = mf[AL] * sqrt_(gi0[0]);
