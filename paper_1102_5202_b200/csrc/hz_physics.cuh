@@ -190,6 +190,17 @@ __device__ __forceinline__ double mc_slope<double>(double qm, double q0, double 
   return s;
 }
 
+// Two MC slopes at once (fp32): differences, doublings and the product packed, min / sign / zero per component.
+__device__ __forceinline__ F2 mc_slope(F2 qm, F2 q0, F2 qp) {
+  const F2 dm = q0 - qm, dp = qp - q0;
+  const F2 dm2 = dm * 2.0f, dp2 = dp * 2.0f, c = (dm + dp) * 0.5f, pr = dm * dp;
+  float sx = fminf(fminf(fabsf(dm2.v.x), fabsf(dp2.v.x)), fabsf(c.v.x));
+  float sy = fminf(fminf(fabsf(dm2.v.y), fabsf(dp2.v.y)), fabsf(c.v.y));
+  sx = dp.v.x > 0 ? sx : -sx;
+  sy = dp.v.y > 0 ? sy : -sy;
+  return F2(pr.v.x <= 0 ? 0.0f : sx, pr.v.y <= 0 ? 0.0f : sy);
+}
+
 // PPM (O4b / R5b): Colella-Woodward edge values on a uniform mesh, built on the
 // monotonised-central slopes above, made monotone, without contact steepening or flattening.
 // Edges of the cell with value q0, from the interface values l, r on its two sides.

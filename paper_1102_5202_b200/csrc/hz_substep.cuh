@@ -224,8 +224,14 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
       ppm_face(a[-2 * sp], a[-sp], a[0], a[sp], a[2 * sp], a[3 * sp], qL[q], qR[q]);
     } else {
       const T qm = a[-sp], q0 = a[0], q1 = a[sp], q2 = a[2 * sp];
-      qL[q] = q0 + T(0.5) * mc_slope(qm, q0, q1);
-      qR[q] = q1 - T(0.5) * mc_slope(q0, q1, q2);
+      if constexpr (sizeof(T) == 4) {  // fp32: the slopes of the two cells as one packed pair
+        const F2 e = F2(q0, q1) + F2(0.5f, -0.5f) * mc_slope(F2(qm, q0), F2(q0, q1), F2(q1, q2));
+        qL[q] = e.v.x;
+        qR[q] = e.v.y;
+      } else {
+        qL[q] = q0 + T(0.5) * mc_slope(qm, q0, q1);
+        qR[q] = q1 - T(0.5) * mc_slope(q0, q1, q2);
+      }
     }
   }
   qL[RHO] = max_(qL[RHO], par.rho_atm); qL[PR] = max_(qL[PR], par.p_atm);
