@@ -74,6 +74,9 @@ def lib():
         L.hzo_get_conserved.argtypes = [C.c_void_p, _dp]
         L.hzo_get_rhs.argtypes = [C.c_void_p, _dp]
         L.hzo_diagnostics.argtypes = [C.c_void_p, C.POINTER(OracleDiag)]
+        L.hzo_set_psi.argtypes = [C.c_void_p, _dp]
+        L.hzo_padded_extent.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.hzo_get_padded.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp]
         L.hzo_strerror.restype = C.c_char_p
         L.hzo_strerror.argtypes = [C.c_int]
         _lib = L
@@ -218,6 +221,20 @@ class Oracle:
         out = np.empty(self._shape(9))
         _chk(lib().hzo_get_rhs(self._h, _p(out)))
         return out
+
+    def set_psi(self, psi):
+        """Test accessor: a manufactured cleaning scalar (the API's prim8 starts it at 0)."""
+        a = _arr(psi, self.ncell)
+        _chk(lib().hzo_set_psi(self._h, _p(a)))
+
+    def get_padded(self, which, field):
+        """Test accessor: one padded array with its ghost layers, shape (Nz, Ny, Nx), and the ghost widths
+        (gx, gy, gz).  which = "prim" (9 fields) or "metric" (10 fields)."""
+        N, g = (C.c_int * 3)(), (C.c_int * 3)()
+        _chk(lib().hzo_padded_extent(self._h, N, g))
+        out = np.empty((N[2], N[1], N[0]))
+        _chk(lib().hzo_get_padded(self._h, {"prim": 0, "metric": 1}[which], int(field), _p(out)))
+        return out, (g[0], g[1], g[2])
 
     def diagnostics(self):
         d = OracleDiag()

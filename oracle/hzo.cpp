@@ -7,7 +7,10 @@
 //
 // Pins (tests/test_oracle_*.py) and what stays "parity unpinned": the CFL choice (R13), the floor
 // thresholds (R11), the face-metric average (R8) and the centred source stencil (R9) are conventions
-// with nothing external to pin them; everything else is pinned as listed in DESIGN.md.
+// with nothing external to pin them; everything else is pinned as listed in DESIGN.md.  The cleaning rows of
+// compute_rhs (flux rows of O2 and the four metric-derivative source terms of O6 / R14) and the ghost fill
+// (O9 / R15) are pinned by tests/test_oracle_cleaning.py: convergence to the non-conservative form of the
+// equations with spectrally exact derivatives on a space-dependent background, and the padded arrays read back.
 #include "hzo.h"
 
 #include <cmath>
@@ -977,6 +980,37 @@ int hzo_get_rhs(hzo_ctx* c, double* rhs9) {
   if (!c->have_prim) return HZO_ESTATE;
   compute_rhs(c);
   return copy_out(c, c->R, rhs9);
+}
+
+// Test accessors (no arithmetic of the method): the cleaning scalar is not part of the API's prim8 (it starts
+// at 0), so the pins of the cleaning rows of compute_rhs set a manufactured psi here; and the ghost-fill pins
+// read one padded array back.
+int hzo_set_psi(hzo_ctx* c, const double* psi) {
+  if (!c || !psi) return HZO_EINVAL;
+  if (!c->have_prim) return HZO_ESTATE;
+  for (int k = 0; k < c->n[2]; k++)
+    for (int j = 0; j < c->n[1]; j++)
+      for (int i = 0; i < c->n[0]; i++) {
+        size_t id = c->idx(i, j, k);
+        double v = psi[((size_t)k * c->n[1] + j) * c->n[0] + i];
+        if (!std::isfinite(v)) return HZO_EINVAL;
+        c->P[8][id] = v;
+        c->U[8][id] = r_val(geometry(met_at(c, id)).sq) * v;
+      }
+  fill_ghosts(c, c->P, NV);
+  return HZO_OK;
+}
+int hzo_padded_extent(const hzo_ctx* c, int* N3, int* g3) {
+  if (!c || !N3 || !g3) return HZO_EINVAL;
+  for (int d = 0; d < 3; d++) { N3[d] = c->N[d]; g3[d] = c->g[d]; }
+  return HZO_OK;
+}
+int hzo_get_padded(hzo_ctx* c, int which, int field, double* out) {   // which: 0 primitives (9), 1 metric (10)
+  if (!c || !out || (which != 0 && which != 1) || field < 0 || field >= (which == 0 ? NV : NM)) return HZO_EINVAL;
+  if (which == 0 ? !c->have_prim : !c->have_metric) return HZO_ESTATE;
+  const std::vector<double>& a = which == 0 ? c->P[field] : c->met[field];
+  for (size_t t = 0; t < c->ncell; t++) out[t] = a[t];
+  return HZO_OK;
 }
 
 // O10.  Diagnostics (PAPER.md:170-174 global reductions): plain loops, long double accumulation.

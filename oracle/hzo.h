@@ -92,6 +92,12 @@ int  hzo_get_psi(hzo_ctx*, double* psi);
 int  hzo_get_conserved(hzo_ctx*, double* cons9);     /* densitised sqrt(gamma)*(D,S,tau,B,psi)  */
 int  hzo_get_rhs(hzo_ctx*, double* rhs9);            /* L(U) for the current primitives         */
 int  hzo_diagnostics(hzo_ctx*, hzo_diag*);
+/* test accessors, no arithmetic: set the cleaning scalar psi (interior planes; U and ghosts follow), read
+ * the padded extents (cells and ghost layers per axis) and one padded array (which: 0 primitives, 1 metric;
+ * x fastest, N[0]*N[1]*N[2] values) */
+int  hzo_set_psi(hzo_ctx*, const double* psi);
+int  hzo_padded_extent(const hzo_ctx*, int* N3, int* g3);
+int  hzo_get_padded(hzo_ctx*, int which, int field, double* out);
 int  hzo_num_threads(void);
 const char* hzo_strerror(int);
 
