@@ -247,7 +247,7 @@ int set_prims_t(hz_ctx* c, const void* prim8) {
   return flag ? HZ_EINVAL : HZ_OK;
 }
 
-template <typename T, int R>
+template <typename T, int R, int FAST>
 int substep_tr(hz_ctx* c, double dt) {
   const Layout& L = c->L;
   const Par<T> par = make_par<T>(c);
@@ -262,12 +262,12 @@ int substep_tr(hz_ctx* c, double dt) {
   {
     ProfScope ps(c, K_SUBSTEP);
     if (sizeof(T) == 4 && c->dtype == HZ_F32_F64)  // fp32 storage and faces, fp64 flux difference / RK / con2prim
-      k_substep<float, double, R><<<grid, G::NT, G::SMEM, c->stream>>>(
+      k_substep<float, double, R, FAST><<<grid, G::NT, G::SMEM, c->stream>>>(
           c->tmP[c->pcur], c->tmM, L, make_par<float>(c), make_par<double>(c), (const float*)c->cln<T>(),
           (const float*)Uin, (const float*)U0,
           (float*)Uout, (float*)c->P<T>(1 - c->pcur), st, dt, c->counters(), ntx, nty, (int)ntiles);
     else
-      k_substep<T, T, R><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, par, c->cln<T>(), Uin, U0, Uout,
+      k_substep<T, T, R, FAST><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, par, c->cln<T>(), Uin, U0, Uout,
                                                             c->P<T>(1 - c->pcur), st, (T)dt, c->counters(), ntx, nty,
                                                             (int)ntiles);
   }
@@ -279,7 +279,9 @@ int substep_tr(hz_ctx* c, double dt) {
 }
 template <typename T>
 int substep_t(hz_ctx* c, double dt) {   // R: reconstruction (0 MC, 1 PPM) -- tile shape and ghost width follow it
-  return c->par.recon == 1 ? substep_tr<T, 1>(c, dt) : substep_tr<T, 0>(c, dt);
+  const bool fast = c->par.cleaning != 0 && c->par.energy_var == 0 && !getenv("HZ_DEBUG_NO_FAST");   // every BASELINE workload
+  if (c->par.recon == 1) return fast ? substep_tr<T, 1, 1>(c, dt) : substep_tr<T, 1, 0>(c, dt);
+  return fast ? substep_tr<T, 0, 1>(c, dt) : substep_tr<T, 0, 0>(c, dt);
 }
 
 // Tensor map of a padded SoA field set as a 4D array (x, y, z, field) with the staging box of k_substep.
@@ -315,8 +317,11 @@ int make_maps_tr(hz_ctx* c) {
   for (int w = 0; w < 2; w++)
     if ((rc = make_tensor_map<T>(c->L, c->P<T>(w), NV, G::BX, G::BY, G::BZ, &c->tmP[w]))) return rc;
   if ((rc = make_tensor_map<T>(c->L, c->met<T>(), NM, G::BX, G::MY, G::MZ, &c->tmM))) return rc;
-  if (cudaFuncSetAttribute(k_substep<T, T, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM) != cudaSuccess ||
-      cudaFuncSetAttribute(k_substep<float, double, R>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  if (cudaFuncSetAttribute(k_substep<T, T, R, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(k_substep<T, T, R, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(k_substep<float, double, R, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)TileGeom<float, R>::SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(k_substep<float, double, R, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)TileGeom<float, R>::SMEM) != cudaSuccess) {
     cudaGetLastError();
     return HZ_ECUDA;

@@ -434,18 +434,23 @@ struct C2P { T D, S2, B2, SB, E; };
 
 template <typename T>
 __device__ __forceinline__ void c2p_eval(T Z, const C2P<T>& c, const Par<T>& par, T& v2, T& f, T& df) {
+  // one reciprocal r = 1/(Z (Z + B^2)) serves 1/Z, 1/(Z + B^2) and their powers; one reciprocal square root
+  // serves sqrt(1 - v^2) and D / (2 sqrt(1 - v^2))
   const T ZB = Z + c.B2;
   const T SB2 = c.SB * c.SB;
   const T Z2 = Z * Z;
-  const T iZ = rcp_(Z), iZB = rcp_(ZB);
-  const T iZ2 = iZ * iZ, iZB2 = iZB * iZB;
-  v2 = (c.S2 * Z2 + SB2 * (c.B2 + 2 * Z)) * iZ2 * iZB2;
+  const T r = rcp_(Z * ZB);
+  const T iZ = ZB * r;
+  const T iZ2 = iZ * iZ;
+  // (the powers of r are applied one factor at a time: r^3 alone overflows fp32 for Z ~ 1e-7)
+  v2 = (c.S2 * Z2 + SB2 * (c.B2 + 2 * Z)) * r * r;
   const T omv = 1 - v2;
-  const T sq = sqrt_(omv);
+  const T rs = rsqrt_(omv);
+  const T sq = omv * rs;
   const T p = par.g1g * (Z * omv - c.D * sq);
   f = Z - p + c.B2 * (1 + v2) * T(0.5) - SB2 * T(0.5) * iZ2 - c.E;
-  const T dv2 = -2 * (c.S2 * Z2 * Z + SB2 * (3 * Z2 + 3 * Z * c.B2 + c.B2 * c.B2)) * (iZ2 * iZ) * (iZB2 * iZB);
-  df = 1 - par.g1g * omv - par.g1g * (-Z + div_(c.D, 2 * sq)) * dv2 + c.B2 * dv2 * T(0.5) + SB2 * iZ2 * iZ;
+  const T dv2 = -2 * (c.S2 * Z2 * Z + SB2 * (3 * Z2 + 3 * Z * c.B2 + c.B2 * c.B2)) * r * r * r;
+  df = 1 - par.g1g * omv - par.g1g * (c.D * rs * T(0.5) - Z) * dv2 + c.B2 * dv2 * T(0.5) + SB2 * iZ2 * iZ;
 }
 
 // w: undensitised conserved; gi: inverse 3-metric (packed); Zg: guess.  Returns 0 on success.

@@ -33,8 +33,13 @@ namespace hz {
 // element of every box row on a 16-byte boundary, so the x halo is 16 bytes: 2 doubles or 4 floats.
 // R = 0: MC-limited linear reconstruction, 2 ghost layers; R = 1: PPM, 3 ghost layers (R5, R5b, R16).
 // PPM's wider halo makes the staged boxes bigger, so its tiles are smaller.
+// NT may exceed the cells of a tile: the extra warps work on the queue of phase 1 only and are the first to
+// start the next tile's queue while the others run the Newton iteration of phase 2.
+#ifndef HZ_NT_D0
+#define HZ_NT_D0 256
+#endif
 template <typename T, int R> struct Tile;
-template <> struct Tile<double, 0> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = 256, HX = 2; };
+template <> struct Tile<double, 0> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = HZ_NT_D0, HX = 2; };
 template <> struct Tile<float, 0> { static constexpr int TX = 16, TY = 8, TZ = 4, NT = 512, HX = 4; };
 template <> struct Tile<double, 1> { static constexpr int TX = 8, TY = 4, TZ = 4, NT = 128, HX = 4; };
 template <> struct Tile<float, 1> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = 256, HX = 4; };
@@ -48,7 +53,7 @@ struct TileGeom {
   static constexpr int NF = NFX + NFY + NFZ;
   static constexpr int WX = (NFX + 31) / 32, WY = (NFY + 31) / 32, WZ = (NFZ + 31) / 32;  // warp items per direction
   // (the last item of a direction may be partly empty)
-  static_assert(NC == NT, "phase 2 maps one cell to one thread");
+  static_assert(NC <= NT && NT % 32 == 0 && NC % 32 == 0, "phase 2 maps one cell to one thread of the first NC");
   static_assert(TY % 4 == 0, "the row swizzle permutes groups of four rows");
   static_assert(HX >= NG && (HX * sizeof(T)) % 16 == 0, "x halo: at least NG cells and 16-byte box rows starts");
   // staged boxes: primitives with halo 2, metric with halo 1; both with halo HX along x (same x origin)
@@ -68,6 +73,15 @@ struct TileGeom {
   static constexpr int NFACE_TASKS = WX + WY + WZ, NSRC_TASKS = NC / 32;  // phase-1 work items (one warp each)
   static constexpr unsigned TX_BYTES = (unsigned)((NV * PFS + NM * MFS) * sizeof(T));
 };
+
+// FAST = 1 instantiates the kernel for the configuration every BASELINE workload runs -- cleaning on, energy slot
+// tau -- with both switches known at compile time; FAST = 0 keeps them run-time (cleaning off, R1b).
+template <int FAST, typename P> __device__ __forceinline__ bool cleaning_(const P& par) {
+  if constexpr (FAST) return true; else return par.cleaning != 0;
+}
+template <int FAST, typename P> __device__ __forceinline__ bool evar_(const P& par) {
+  if constexpr (FAST) return false; else return par.energy_var != 0;
+}
 
 // packed index of gamma_{(d+a)%3, (d+b)%3} for (a,b) = 00 01 02 11 12 22
 __device__ __forceinline__ int rot6(int d, int a) {
@@ -184,11 +198,66 @@ __device__ __forceinline__ void state_flux0(const T* q, const S* m, const S* gi0
   lm = aod * (vd - sq) - be;
 }
 
+// ---- the same state in the fast mode (cleaning on, energy slot = tau): its share of the HLLE flux ------
+// With cleaning on the signal speeds of a face are the light cone of the (B^d, psi) subsystem: the fluid's
+// fast-speed bound of O3 is the coordinate speed of a signal that moves with a <= 1 in the fluid frame, so it
+// never leaves that cone, and max / min with it return the cone itself ("light-cone
+// speeds").  The HLLE weights then depend on the face metric only, the flux is linear in (U, F) of each
+// side with known weights, and each state adds  C = cF F + cU U  without U, F or the fluid speeds ever
+// existing as vectors: with k = cF vt + cU every advected row is (row of U) * k plus its pressure / field term.
+template <typename T, typename S>
+__device__ __forceinline__ void state_contrib0(const T* q, const S* m, const S* gi0, const Par<S>& par, T cF, T cU,
+                                               T* C) {
+  const S* g = m + GXX;
+  T utl[3], Bl[3];
+  lower(g, q + UX, utl);
+  lower(g, q + BX, Bl);
+  const T ut2 = dot3(q + UX, utl);
+  const T W2 = 1 + ut2;
+  const T iW = rsqrt_(W2);
+  const T W = W2 * iW;
+  const T iW2 = iW * iW;
+  const T v2 = ut2 * iW2;
+  const T rhoh = q[RHO] + par.gg1 * q[PR];
+  const T B2 = dot3(q + BX, Bl);
+  const T Bv = dot3(q + BX, utl) * iW;
+  const T Bv2 = Bv * Bv;
+  const T b2 = B2 * iW2 + Bv2;
+  const T Z = rhoh * W2;
+  const T D = q[RHO] * W;
+  const T ZB = Z + B2;
+  const S al = m[AL], be = m[BEX];
+  const T v0 = q[UX] * iW;
+  const T k = cF * (al * v0 - be) + cU;
+  const T B0 = q[BX];
+  const T aBd = al * B0 * iW;   // alpha B^0 / W
+  const T cFa = cF * aBd;
+  const T WBv = W * Bv;
+  const T cap = cF * (al * (q[PR] + b2 * T(0.5)));   // cF alpha p*
+  C[0] = D * k;
+#pragma unroll
+  for (int j = 0; j < 3; j++) {
+    const T vlj = utl[j] * iW;
+    const T Sj = ZB * vlj - Bv * Bl[j];
+    const T bj = Bl[j] * iW + WBv * vlj;
+    C[1 + j] = Sj * k - cFa * bj;
+  }
+  C[1] = C[1] + cap;
+  const T tau = Z - q[PR] + (B2 * (1 + v2) - Bv2) * T(0.5) - D;
+  C[4] = tau * k + cap * v0 - cFa * WBv;   // alpha Bv B^0 = (alpha B^0 / W) (W Bv)
+  const T psi = q[PSI];
+  const T capsi = cF * (al * psi);
+  C[5] = capsi * gi0[0] + (cU - cF * be) * B0;
+#pragma unroll
+  for (int c = 1; c < 3; c++) C[5 + c] = q[BX + c] * k + capsi * gi0[c] - cFa * q[UX + c];
+  C[8] = cF * (al * B0 - be * psi) + cU * psi;
+}
+
 // ---- a1-a4 for one face of a sweep along axis d, everything read from the staged tile ---------------
 // sPc / sMc: staged primitives / metric at the cell on the MINUS side of the face (field 0);
 // sp / sm: element stride of axis d inside the two boxes.
 // Phi comes out in the sweep frame: Phi[1+a] belongs to S_{(d+a)%3}, Phi[5+a] to B^{(d+a)%3}.
-template <typename T, int R>
+template <typename T, int R, int FAST>
 __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T* __restrict__ sMc, int sp, int sm,
                                               int d, const Par<T>& par, T* Phi) {
   using G = TileGeom<T, R>;
@@ -236,6 +305,28 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
   }
   qL[RHO] = max_(qL[RHO], par.rho_atm); qL[PR] = max_(qL[PR], par.p_atm);
   qR[RHO] = max_(qR[RHO], par.rho_atm); qR[PR] = max_(qR[PR], par.p_atm);
+  if constexpr (FAST) {
+    // cleaning on: the light cone bounds every signal, so the HLLE weights are functions of the face metric
+    const T c = mf[AL] * sqrt_(gi0[0]);
+    const T lp = max_(c - mf[BEX], T(0)), lm = min_(-c - mf[BEX], T(0));
+    const T sw = div_(sqg, lp - lm);           // lp - lm >= 2 c > 0
+    const T cFL = sw * lp, cFR = -(sw * lm), cUU = sw * lp * lm;
+    if constexpr (sizeof(T) == 4) {  // fp32: both states as one packed stream
+      F2 q2[NV], C2[NV];
+#pragma unroll
+      for (int v = 0; v < NV; v++) q2[v] = F2(qL[v], qR[v]);
+      state_contrib0(q2, mf, gi0, par, F2(cFL, cFR), F2(-cUU, cUU), C2);
+#pragma unroll
+      for (int v = 0; v < NV; v++) Phi[v] = C2[v].v.x + C2[v].v.y;
+    } else {
+      T CR[NV];
+      state_contrib0(qL, mf, gi0, par, cFL, -cUU, Phi);
+      state_contrib0(qR, mf, gi0, par, cFR, cUU, CR);
+#pragma unroll
+      for (int v = 0; v < NV; v++) Phi[v] += CR[v];
+    }
+    return;
+  }
   T UL[NV], FL[NV], UR[NV], FR[NV], lmL, lpL, lmR, lpR;
   if constexpr (sizeof(T) == 4) {  // fp32: both states as one packed stream (F2, hz_physics.cuh)
     F2 q2[NV], U2[NV], Fx2[NV], lm2, lp2;
@@ -271,7 +362,7 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
 
 // ---- a6 from the staged metric: centred differences, fluid and cleaning sources at a cell ----------
 // sMc: staged metric at the cell (field 0).  Same arithmetic as add_sources (hz_kernels.cuh).
-template <typename T, int R>
+template <typename T, int R, int FAST>
 __device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __restrict__ sMc, const T* m, const T* q,
                                                    const Par<T>& par, const T* gi, T sq, const T* cl4, T* Rs) {
   using G = TileGeom<T, R>;
@@ -294,7 +385,7 @@ __device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __r
     for (int a = 0; a < NM; a++) dm[d][a] = (mp[a] - mm[a]) * i2h;
   }
   fluid_source(q, m, dm, par, gi, sq, Rs);
-  if (par.cleaning) {  // cleaning sources (R14), not multiplied by alpha
+  if (cleaning_<FAST>(par)) {  // cleaning sources (R14), not multiplied by alpha
 #pragma unroll
     for (int k = 0; k < 3; k++) {
       const T adv = q[BX] * dm[0][BEX + k] + q[BY] * dm[1][BEX + k] + q[BZ] * dm[2][BEX + k];
@@ -365,7 +456,7 @@ __device__ __forceinline__ int cdiv(int n) {
 
 // ---- the work items of phase 1 ----------------------------------------------------------------------
 // Face item: 32 consecutive faces of one direction -> Phi into sF.
-template <typename T, int R>
+template <typename T, int R, int FAST>
 __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, const T* sP, const T* sM, T* sF, int task,
                                           int lane, int x0, int y0, int z0) {
   using G = TileGeom<T, R>;
@@ -393,7 +484,7 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
   const T* sPc = sP + ((c + G::NG) * G::BY + (b + G::NG)) * G::BX + (a + G::HX) - sp;
   const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX) - sm;
   T Phi[NV];
-  face_flux_rot<T, R>(sPc, sMc, sp, sm, d, par, Phi);
+  face_flux_rot<T, R, FAST>(sPc, sMc, sp, sm, d, par, Phi);
   T* o = sF + off + (c * e1 + b) * e0 + a;
   o[0] = Phi[0];
   o[4 * G::NF] = Phi[4];
@@ -408,7 +499,7 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
 
 // Source item: the geometric and cleaning sources (a6) of 32 cells -> sR[(q-1) * NC + cell], q = 1..8
 // (the D equation has no source).  Needs no flux, so it fills the scheduling gaps of the face items.
-template <typename T, int R>
+template <typename T, int R, int FAST>
 __device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, const T* sP, const T* sM, T* sR,
                                             const T* __restrict__ cln, int cell, int x0, int y0, int z0) {
   using G = TileGeom<T, R>;
@@ -432,13 +523,13 @@ __device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, 
 #pragma unroll
   for (int v = 0; v < NV; v++) Rs[v] = 0;
   T cl4[4] = {0, 0, 0, 0};
-  if (par.cleaning) {
+  if (cleaning_<FAST>(par)) {
     const long long id = L.idx(x0 + a, y0 + b, z0 + c);
 #pragma unroll
     for (int v = 0; v < 4; v++) cl4[v] = cln[v * L.fs + id];
   }
-  add_sources_staged<T, R>(L, sMc, m, q, par, gi, sq, cl4, Rs);
-  if (par.energy_var) Rs[4] = 0;  // R1b: no source on a fixed metric
+  add_sources_staged<T, R, FAST>(L, sMc, m, q, par, gi, sq, cl4, Rs);
+  if (evar_<FAST>(par)) Rs[4] = 0;  // R1b: no source on a fixed metric
 #pragma unroll
   for (int v = 1; v < NV; v++) sR[(v - 1) * G::NC + cell] = Rs[v];
 }
@@ -458,17 +549,18 @@ __device__ __forceinline__ void issue_loads(const CUtensorMap* tmP, const CUtens
 
 // ---- the kernel: persistent blocks, one tile per iteration ----------------------------------------
 // stage 0: Uout = Uin + dt L;  1: Uout = 3/4 U0 + 1/4 (Uin + dt L);  2: Uout = 1/3 U0 + 2/3 (Uin + dt L)
+// Uin and Uout are the SAME buffer in stages 1 and 2 (no __restrict__ on them): the update is in place, which is
+// safe because a thread reads only its own cell of U, once, before it writes it.
 // tmP / tmM: tensor maps of the current primitives and of the metric as 4D arrays (x, y, z, field).
 // Tiles are numbered x fastest; block b takes tiles b, b + gridDim.x, ...  While a block is in phase 2
 // of one tile, the TMA loads of its next tile are already in flight (the staged boxes are dead by then).
 // T2 is the arithmetic type of phase 2.  T2 = T: pure fp64 or pure fp32.  T = float with
 // T2 = double is the paper's mixed mode: storage, reconstruction and face fluxes in
 // fp32; flux difference, Runge-Kutta combine and the primitive recovery in fp64.
-template <typename T, typename T2, int R>
+template <typename T, typename T2, int R, int FAST>
 __global__ void __launch_bounds__(Tile<T, R>::NT, 1)
 k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmM, Layout L, Par<T> par,
-          Par<T2> par2, const T* __restrict__ cln, const T* __restrict__ Uin, const T* __restrict__ U0,
-          T* __restrict__ Uout,
+          Par<T2> par2, const T* __restrict__ cln, const T* Uin, const T* __restrict__ U0, T* Uout,
           T* __restrict__ Pout, int stage, T2 dt, unsigned long long* __restrict__ counters, int ntx, int nty,
           int ntiles) {
   using G = TileGeom<T, R>;
@@ -489,7 +581,9 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
   if (threadIdx.x == 0 && (int)blockIdx.x < ntiles) issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, blockIdx.x, ntx, nty);
 
   // this thread's cell of phase 2 (one cell per thread), tile-local
-  const int ca = threadIdx.x % G::TX, cr = threadIdx.x / G::TX;
+  const bool has_cell = G::NT == G::NC || (int)threadIdx.x < G::NC;   // warp-uniform
+  const int ctid = has_cell ? (int)threadIdx.x : 0;
+  const int ca = ctid % G::TX, cr = ctid / G::TX;
   const int cb = swz(cr % G::TY), cc = cr / G::TY;
   const T* sPc = sP + ((cc + G::NG) * G::BY + (cb + G::NG)) * G::BX + (ca + G::HX);
   const T* sMc = sM + ((cc + 1) * G::MY + (cb + 1)) * G::BX + (ca + G::HX);
@@ -501,7 +595,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     const int tx = tile % ntx, tr = tile / ntx;
     const int x0 = tx * G::TX, y0 = (tr % nty) * G::TY, z0 = (tr / nty) * G::TZ;
     const int ci = x0 + ca, cj = y0 + cb, ck = z0 + cc;
-    const bool cell_ok = ci < L.n[0] && cj < L.n[1] && ck < L.n[2];
+    const bool cell_ok = has_cell && ci < L.n[0] && cj < L.n[1] && ck < L.n[2];
     const long long id = L.idx(ci, cj, ck);
     mbar_wait(bar, parity);
 
@@ -515,24 +609,29 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       const int t = __shfl_sync(0xffffffffu, fetched, 0);
       if (t >= G::NFACE_TASKS + G::NSRC_TASKS) break;
       if (lane == 0) fetched = atomicAdd(queue, 1);
-      if (t < G::NFACE_TASKS) face_task<T, R>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
-      else source_task<T, R>(L, par, sP, sM, sR, cln, (t - G::NFACE_TASKS) * 32 + lane, x0, y0, z0);
+      if (t < G::NFACE_TASKS) face_task<T, R, FAST>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
+      else source_task<T, R, FAST>(L, par, sP, sM, sR, cln, (t - G::NFACE_TASKS) * 32 + lane, x0, y0, z0);
     }
-    // inputs of this thread's cell: conserved state from HBM (latency overlaps the barrier wait),
-    // previous primitives and metric from the staged boxes (free for the next tile afterwards)
-    T u[NV], u0[NV], q[NV], m[NM];
+    // inputs of this thread's cell: conserved state from HBM (latency overlaps the barrier wait), metric and
+    // the Newton guess Z = rho h W^2 of the previous primitives from the staged boxes (free for the next
+    // tile afterwards)
+    T u[NV], m[NM];
+    T2 Zg = 0;
     if (cell_ok) {
 #pragma unroll
       for (int v = 0; v < NV; v++) u[v] = Uin[v * L.fs + id];
-      if (stage != 0) {
-#pragma unroll
-        for (int v = 0; v < NV; v++) u0[v] = U0[v * L.fs + id];
-      }
     }
+    if (has_cell) {
 #pragma unroll
-    for (int v = 0; v < NV; v++) q[v] = sPc[v * G::PFS];
+      for (int v = 0; v < NM; v++) m[v] = sMc[v * G::MFS];
+      T2 ut[3], utl[3], g2[6];
 #pragma unroll
-    for (int v = 0; v < NM; v++) m[v] = sMc[v * G::MFS];
+      for (int a3 = 0; a3 < 3; a3++) ut[a3] = (T2)sPc[(UX + a3) * G::PFS];
+#pragma unroll
+      for (int a6 = 0; a6 < 6; a6++) g2[a6] = (T2)m[GXX + a6];
+      lower(g2, ut, utl);
+      Zg = ((T2)sPc[RHO * G::PFS] + par2.gg1 * (T2)sPc[PR * G::PFS]) * (1 + dot3(ut, utl));
+    }
     __syncthreads();  // all fluxes and sources are in shared memory; nobody reads sP / sM any more
     if (threadIdx.x == 0) {
       *queue = 0;
@@ -540,14 +639,21 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     }
 
     // ---- phase 2: one cell per thread, arithmetic in T2 ----
-    // 2a: right-hand side from the fluxes and sources in shared memory; after the barrier below sF / sR are
-    // free, so a warp that finishes 2b early goes straight on to the next tile's work queue (the Newton
-    // iteration counts differ from cell to cell, and no barrier follows them).
-    T2 Rh[NV];
+    // 2a: right-hand side from the fluxes and sources in shared memory and the Euler stage u + dt L; after the
+    // barrier below sF / sR are free, so a warp that finishes 2b early goes straight on to the next tile's work
+    // queue (the Newton iteration counts differ from cell to cell, and no barrier follows them).  The state at
+    // the start of the step (stages 1, 2) is requested here and used after the barrier.
+    T2 un[NV];
+    T u0[NV];
     if (cell_ok) {
+      if (stage != 0) {
+#pragma unroll
+        for (int v = 0; v < NV; v++) u0[v] = U0[v * L.fs + id];
+      }
+      T2 Rh[NV];
       Rh[0] = 0;
 #pragma unroll
-      for (int v = 1; v < NV; v++) Rh[v] = (T2)sR[(v - 1) * G::NC + threadIdx.x];
+      for (int v = 1; v < NV; v++) Rh[v] = (T2)sR[(v - 1) * G::NC + ctid];
       if (L.g[0]) {
         const T2 ih = par2.ih[0];
         const T* o = sF + (cc * G::TY + cb) * (G::TX + 1) + ca;
@@ -566,25 +672,22 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
 #pragma unroll
         for (int v = 0; v < NV; v++) Rh[v] -= ((T2)o[v * G::NF + G::TX * G::TY] - (T2)o[v * G::NF]) * ih;
       }
-      if (!par2.cleaning) Rh[8] = 0;
+      if (!cleaning_<FAST>(par2)) Rh[8] = 0;
+#pragma unroll
+      for (int v = 0; v < NV; v++) un[v] = (T2)u[v] + dt * Rh[v];
     }
     __syncthreads();  // everybody has read sF / sR: the next tile's phase 1 may overwrite them
     if (cell_ok) {  // 2b
       // a7: Runge-Kutta stage combine
-      T2 un[NV];
+      if (stage != 0) {
+        const T2 wa = stage == 1 ? T2(0.75) : T2(1.0 / 3.0), wb = stage == 1 ? T2(0.25) : T2(2.0 / 3.0);
 #pragma unroll
-      for (int v = 0; v < NV; v++) {
-        T2 u1 = (T2)u[v] + dt * Rh[v];
-        if (stage == 1) u1 = T2(0.75) * (T2)u0[v] + T2(0.25) * u1;
-        if (stage == 2) u1 = T2(1.0 / 3.0) * (T2)u0[v] + T2(2.0 / 3.0) * u1;
-        un[v] = u1;
+        for (int v = 0; v < NV; v++) un[v] = wa * (T2)u0[v] + wb * un[v];
       }
       // a8: primitive recovery and floors
-      T2 m2[NM], q2[NV];
+      T2 m2[NM];
 #pragma unroll
       for (int v = 0; v < NM; v++) m2[v] = (T2)m[v];
-#pragma unroll
-      for (int v = 0; v < NV; v++) q2[v] = (T2)q[v];
       T2 cf[6], gi[6];
       const T2 det = cofactors(m2 + GXX, cf);
       const T2 sq = sqrt_(det);
@@ -595,15 +698,8 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       T2 w[NV];
 #pragma unroll
       for (int v = 0; v < NV; v++) w[v] = un[v] * isq;
-      if (!par2.cleaning) w[8] = 0;
-      if (par2.energy_var) w[4] = energy_to_tau(w, m2);
-      T2 Zg;
-      {  // guess from the previous primitives of this cell
-        T2 utl[3];
-        lower(m2 + GXX, q2 + UX, utl);
-        const T2 W2 = 1 + dot3(q2 + UX, utl);
-        Zg = (q2[RHO] + par2.gg1 * q2[PR]) * W2;
-      }
+      if (!cleaning_<FAST>(par2)) w[8] = 0;
+      if (evar_<FAST>(par2)) w[4] = energy_to_tau(w, m2);
       T2 qn[NV];
       int its = 0;
       const int fl = con2prim(w, m2, gi, par2, Zg, qn, its);
@@ -623,7 +719,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       if (rs || pf) {
         T2 uf[NV];
         prim2con(qn, m2, par2, uf);
-        if (par2.energy_var) uf[4] = tau_to_energy(uf, m2);
+        if (evar_<FAST>(par2)) uf[4] = tau_to_energy(uf, m2);
 #pragma unroll
         for (int v = 0; v < NV; v++) un[v] = sq * uf[v];
       }
