@@ -61,13 +61,33 @@ __device__ __forceinline__ float div_(float a, float b) {
   asm("div.approx.f32 %0, %1, %2;" : "=f"(q) : "f"(a), "f"(b));
   return q;
 }
-__device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+// fp64 reciprocal square root and square root of a POSITIVE, finite, normal argument (Lorentz factors, metric
+// determinants, 1 - v^2 of an accepted Newton trial): hardware seed (MUFU.RSQ64H, >= 20 bits) + one third-order
+// step (relative error ~1e-18 before rounding), and for the root one residual correction.  No special cases: a
+// zero or negative argument gives inf / NaN, which the callers' finite checks treat as a failed trial.  The
+// library routines (sqrt, rsqrt) spend twice the instructions on the cases that cannot occur here.
+__device__ __forceinline__ double rsqrt_(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double t = x * y;
+  const double e = fma(-t, y, 1.0);
+  const double p = fma(0.375, e, 0.5);
+  return fma(y * e, p, y);
+}
+__device__ __forceinline__ double sqrt_(double x) {
+  const double y = rsqrt_(x);
+  const double s = x * y;
+  const double r = fma(-s, s, x);
+  return fma(r * 0.5, y, s);
+}
+// square root of an argument that may be exactly zero
+__device__ __forceinline__ double sqrt0_(double x) { return sqrt(x); }
 __device__ __forceinline__ float sqrt_(float x) {
   float y;
   asm("sqrt.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-__device__ __forceinline__ double rsqrt_(double x) { return rsqrt(x); }
+__device__ __forceinline__ float sqrt0_(float x) { return sqrt_(x); }
 __device__ __forceinline__ float rsqrt_(float x) {
   float y;
   asm("rsqrt.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -109,6 +129,7 @@ __device__ __forceinline__ F2 operator*(F2 a, float b) { return a * F2(b); }
 __device__ __forceinline__ F2& operator+=(F2& a, F2 b) { a = a + b; return a; }
 __device__ __forceinline__ F2 rsqrt_(F2 a) { return F2(rsqrt_(a.v.x), rsqrt_(a.v.y)); }
 __device__ __forceinline__ F2 sqrt_(F2 a) { return F2(sqrt_(a.v.x), sqrt_(a.v.y)); }
+__device__ __forceinline__ F2 sqrt0_(F2 a) { return sqrt_(a); }
 __device__ __forceinline__ F2 rcp_(F2 a) { return F2(rcp_(a.v.x), rcp_(a.v.y)); }
 __device__ __forceinline__ F2 div_(F2 a, F2 b) { return a * rcp_(b); }
 __device__ __forceinline__ F2 div_(float a, F2 b) { return F2(a) * rcp_(b); }
@@ -321,7 +342,7 @@ __device__ __forceinline__ void flux_speeds(const T* q, const T* m, const T* gid
   a2 = min_(max_(a2, T(0)), T(1));
   T den = 1 - s.v2 * a2;
   T disc = a2 * (1 - s.v2) * (den * gid[D] - (1 - a2) * s.v[D] * s.v[D]);
-  T sq = sqrt_(max_(disc, T(0)));
+  T sq = sqrt0_(max_(disc, T(0)));
   T aod = div_(al, den);
   T vd = s.v[D] * (1 - a2);
   lp = aod * (vd + sq) - be;
