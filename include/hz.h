@@ -67,7 +67,11 @@ typedef struct {
   double kappa;           /* cleaning damping rate                                              */
   int    c2p_maxit;       /* Newton iteration cap of the primitive recovery                     */
   double c2p_tol;         /* converged when |dZ| <= c2p_tol*Z; <= 0 selects the dtype default   */
-                          /* (1e-13 for HZ_F64, 1e-6 for HZ_F32)                                */
+                          /* (1e-13 for HZ_F64, 1e-6 for HZ_F32, 1e-10 for the fp64 recovery of */
+                          /* HZ_F32_F64).  HZ_F32 measures the step against Z + B^2 (the round- */
+                          /* off of the residual is eps*(Z + B^2)) and also accepts a step that  */
+                          /* has stopped shrinking below 64 eps of that scale (counted in        */
+                          /* hz_diag.c2p_stalled); no other acceptance exists                    */
   int    c2p_scheme;      /* 0: Newton on Z = rho h W^2; 1: Newton on the two unknowns (Z, v^2),  */
                           /* the paper's second recovery scheme.  Same root.       */
   int    energy_var;      /* 0: the energy slot of U is sqrt(gamma) tau (north_star); 1: the paper's */
@@ -86,6 +90,8 @@ typedef struct {
   double max_speed_over_dx;                  /* max over cells, axes of max(|lam+|,|lam-|)/dx_d       */
   long long c2p_fail, atm_reset, p_floor;    /* cumulative since hz_set_primitives                    */
   int c2p_maxit_seen;
+  long long c2p_stalled;                     /* HZ_F32 only: recoveries accepted by the round-off rule */
+                                             /* of c2p_tol below (not failures; cumulative)            */
 } hz_diag;
 
 /* Fill *p with the defaults: Gamma = 4/3, atmosphere 1e-12 / 1e-14, atm_tol 1e-3, cleaning on,

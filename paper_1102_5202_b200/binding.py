@@ -44,7 +44,7 @@ class HzDiag(C.Structure):
                 ("sumTau", C.c_double), ("sumBx", C.c_double), ("sumBy", C.c_double), ("sumBz", C.c_double),
                 ("sumPsi", C.c_double), ("divB_max", C.c_double), ("divB_L1", C.c_double),
                 ("max_speed_over_dx", C.c_double), ("c2p_fail", C.c_longlong), ("atm_reset", C.c_longlong),
-                ("p_floor", C.c_longlong), ("c2p_maxit_seen", C.c_int)]
+                ("p_floor", C.c_longlong), ("c2p_maxit_seen", C.c_int), ("c2p_stalled", C.c_longlong)]
 
     def asdict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

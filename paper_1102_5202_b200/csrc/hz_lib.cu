@@ -74,7 +74,7 @@ Plan make_plan(const Layout& L, int dtype) {
   p.diag_blocks = (int)(nb < 1184 ? nb : 1184);  // 148 SMs x 8 resident blocks
   p.partials = take((size_t)p.diag_blocks * NDIAG * sizeof(double));
   p.diag_out = take(NDIAG * sizeof(double));
-  p.counters = take(4 * sizeof(unsigned long long));
+  p.counters = take(8 * sizeof(unsigned long long));
   p.err = take(sizeof(int));
   p.total = o;
   return p;
@@ -235,7 +235,7 @@ int set_prims_t(hz_ctx* c, const void* prim8) {
   int rc;
   if ((rc = to_device<T>(c, prim8, 8 * n, c->staging<T>(), &p))) return rc;
   HZ_CUDA(cudaMemsetAsync(c->err(), 0, sizeof(int), c->stream));
-  HZ_CUDA(cudaMemsetAsync(c->counters(), 0, 4 * sizeof(unsigned long long), c->stream));
+  HZ_CUDA(cudaMemsetAsync(c->counters(), 0, 8 * sizeof(unsigned long long), c->stream));
   c->cur = 0; c->u0 = 1; c->pcur = 0; c->stage = 0;
   k_pack_prims<T><<<nblocks(n, 128), 128, 0, c->stream>>>(L, make_par<T>(c), p, c->met<T>(), c->P<T>(0), c->U<T>(0),
                                                           c->err());
@@ -371,7 +371,7 @@ int diag_t(hz_ctx* c, hz_diag* out) {
   k_diag_final<<<1, 32, 0, c->stream>>>(c->partials(), nb, c->diag_out());
   HZ_LAUNCHED(c);
   double h[12];
-  unsigned long long cnt[4];
+  unsigned long long cnt[8];
   HZ_CUDA(cudaMemcpyAsync(h, c->diag_out(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   HZ_CUDA(cudaMemcpyAsync(cnt, c->counters(), sizeof(cnt), cudaMemcpyDeviceToHost, c->stream));
   HZ_CUDA(cudaStreamSynchronize(c->stream));
@@ -384,6 +384,7 @@ int diag_t(hz_ctx* c, hz_diag* out) {
   out->max_speed_over_dx = h[11];
   out->c2p_fail = (long long)cnt[0]; out->atm_reset = (long long)cnt[1]; out->p_floor = (long long)cnt[2];
   out->c2p_maxit_seen = (int)cnt[3];
+  out->c2p_stalled = (long long)cnt[4];
   return HZ_OK;
 }
 

@@ -474,9 +474,22 @@ __device__ __forceinline__ void c2p_eval(T Z, const C2P<T>& c, const Par<T>& par
   df = 1 - par.g1g * omv - par.g1g * (c.D * rs * T(0.5) - Z) * dv2 + c.B2 * dv2 * T(0.5) + SB2 * iZ2 * iZ;
 }
 
-// w: undensitised conserved; gi: inverse 3-metric (packed); Zg: guess.  Returns 0 on success.
+// v^2(Z) alone: what the accepted last step still needs (its f and f' would never be used)
 template <typename T>
-__device__ __forceinline__ int con2prim_1d(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters) {
+__device__ __forceinline__ T c2p_v2(T Z, const C2P<T>& c) {
+  const T r = rcp_(Z * (Z + c.B2));
+  return (c.S2 * Z * Z + c.SB * c.SB * (c.B2 + 2 * Z)) * r * r;
+}
+// fp32 only: the residual f carries a round-off of eps (Z + B^2), so the Newton step cannot shrink below a few
+// eps of that scale.  A step that has stopped shrinking while it is below STALL_EPS machine epsilons of the scale
+// has found the root to working precision: it is accepted, counted (hz_diag.c2p_stalled) and the iteration ends.
+constexpr float C2P_STALL_EPS = 64.0f * 1.1920929e-7f;
+
+// w: undensitised conserved; gi: inverse 3-metric (packed); Zg: guess.  Returns 0 on success, 1 on failure;
+// `stalled` is set when the fp32 round-off rule above ended the iteration.
+template <typename T>
+__device__ __forceinline__ int con2prim_1d(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters,
+                                           int& stalled) {
   C2P<T> c;
   T Su[3], Bl[3];
   lower(gi, w + 1, Su);
@@ -500,10 +513,16 @@ __device__ __forceinline__ int con2prim_1d(const T* w, const T* m, const T* gi, 
   }
   if (!(v2 < 1)) return 1;
   bool ok = false;
-  T dZ = Z;
+  T dZ = Z, dZprev = Z;
   for (int it = 1; it <= par.c2p_maxit; it++) {
     iters = it;
     T Zn = Z - div_(f, df);
+    // fp64: |dZ| <= tol Z (R11).  fp32: the test is made against Z + B^2 (see C2P_STALL_EPS).
+    // A step that already meets the tolerance is the last one: only v^2 at the new point is still needed.
+    if (finite_(Zn) && Zn > 0 && abs_(Zn - Z) <= par.c2p_tol * (sizeof(T) == 4 ? Zn + c.B2 : Zn)) {
+      const T v2n = c2p_v2(Zn, c);
+      if (v2n < 1) { Z = Zn; v2 = v2n; ok = true; break; }
+    }
     T v2n, fn, dfn;
     int halv = 0;
     for (;;) {  // keep Z > 0 and v^2 < 1 by halving the step
@@ -516,16 +535,13 @@ __device__ __forceinline__ int con2prim_1d(const T* w, const T* m, const T* gi, 
       if (++halv > 40) return 1;
       Zn = (Z + Zn) * T(0.5);
     }
+    dZprev = dZ;
     dZ = abs_(Zn - Z);
     Z = Zn; v2 = v2n; f = fn; df = dfn;
-    // fp64: |dZ| <= tol Z (R11).  fp32: the round-off of f is eps * (Z + B^2), so where the field
-    // dominates (B^2 > Z) the step cannot fall below that; the test is made against Z + B^2 there.
     const T scale = sizeof(T) == 4 ? Z + c.B2 : Z;
-    if (dZ <= par.c2p_tol * scale) { ok = true; break; }
+    if (dZ <= par.c2p_tol * scale) { ok = true; break; }   // (a halved step that lands within the tolerance)
+    if (sizeof(T) == 4 && it >= 2 && dZ >= dZprev && dZ <= T(C2P_STALL_EPS) * scale) { ok = true; stalled = 1; break; }
   }
-  // fp32 only: an iteration that has stalled at the round-off floor (last step below 1e-4 of the scale) has
-  // found the root to working precision; resetting such a cell to atmosphere would be the larger error.
-  if (!ok && sizeof(T) == 4 && dZ <= T(1e-4) * (Z + c.B2)) ok = true;
   if (!ok) return 1;
   const T omv = 1 - v2;
   const T sq = sqrt_(omv);
@@ -547,7 +563,8 @@ __device__ __forceinline__ int con2prim_1d(const T* w, const T* m, const T* gi, 
 // ---- O8b: the same root by Newton on the two unknowns (Z, v^2) ("2D_W"; R10b) ----
 //   g1 = v2 - V(Z),  g2 = Z - p(Z, v2) + B^2 (1 + v2)/2 - SB^2/(2 Z^2) - E,  Jacobian [[-V', 1], [a, b]]
 template <typename T>
-__device__ __forceinline__ int con2prim_2d(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters) {
+__device__ __forceinline__ int con2prim_2d(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters,
+                                           int& stalled) {
   C2P<T> c;
   T Su[3], Bl[3];
   lower(gi, w + 1, Su);
@@ -571,7 +588,7 @@ __device__ __forceinline__ int con2prim_2d(const T* w, const T* m, const T* gi, 
   if (!(v2 < 1)) return 1;
   const T SB2 = c.SB * c.SB;
   bool ok = false;
-  T dZ = Z, dv = 1;
+  T dZ = Z, dv = 1, dZprev = Z;
   for (int it = 1; it <= par.c2p_maxit; it++) {
     iters = it;
     const T ZB = Z + c.B2, Z2 = Z * Z;
@@ -607,8 +624,10 @@ __device__ __forceinline__ int con2prim_2d(const T* w, const T* m, const T* gi, 
     Z = Zn; v2 = vn;
     const T scale = sizeof(T) == 4 ? Z + c.B2 : Z;   // fp32: see con2prim_1d
     if (abs_(dZ) <= par.c2p_tol * scale && abs_(dv) <= par.c2p_tol) { ok = true; break; }
+    if (sizeof(T) == 4 && it >= 2 && abs_(dZ) >= dZprev && abs_(dZ) <= T(C2P_STALL_EPS) * scale &&
+        abs_(dv) <= T(C2P_STALL_EPS)) { ok = true; stalled = 1; break; }
+    dZprev = abs_(dZ);
   }
-  if (!ok && sizeof(T) == 4 && abs_(dZ) <= T(1e-4) * (Z + c.B2) && abs_(dv) <= T(1e-4)) ok = true;
   if (!ok) return 1;
   const T omv = 1 - v2;
   const T sq = sqrt_(omv);
@@ -628,9 +647,10 @@ __device__ __forceinline__ int con2prim_2d(const T* w, const T* m, const T* gi, 
 }
 
 template <typename T>
-__device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters) {
-  if (par.c2p_scheme == 1) return con2prim_2d(w, m, gi, par, Zg, q, iters);   // uniform over the launch
-  return con2prim_1d(w, m, gi, par, Zg, q, iters);
+__device__ __forceinline__ int con2prim(const T* w, const T* m, const T* gi, const Par<T>& par, T Zg, T* q, int& iters,
+                                        int& stalled) {
+  if (par.c2p_scheme == 1) return con2prim_2d(w, m, gi, par, Zg, q, iters, stalled);   // uniform over the launch
+  return con2prim_1d(w, m, gi, par, Zg, q, iters, stalled);
 }
 
 }  // namespace hz

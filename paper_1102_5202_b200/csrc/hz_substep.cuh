@@ -37,11 +37,17 @@ namespace hz {
 #ifndef HZ_NT_D0
 #define HZ_NT_D0 256
 #endif
+#ifndef HZ_NT_D1
+#define HZ_NT_D1 256
+#endif
+#ifndef HZ_NT_F1
+#define HZ_NT_F1 512
+#endif
 template <typename T, int R> struct Tile;
 template <> struct Tile<double, 0> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = HZ_NT_D0, HX = 2; };
 template <> struct Tile<float, 0> { static constexpr int TX = 16, TY = 8, TZ = 4, NT = 512, HX = 4; };
-template <> struct Tile<double, 1> { static constexpr int TX = 8, TY = 4, TZ = 4, NT = 128, HX = 4; };
-template <> struct Tile<float, 1> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = 256, HX = 4; };
+template <> struct Tile<double, 1> { static constexpr int TX = 8, TY = 4, TZ = 4, NT = HZ_NT_D1, HX = 4; };
+template <> struct Tile<float, 1> { static constexpr int TX = 8, TY = 8, TZ = 4, NT = HZ_NT_F1, HX = 4; };
 
 template <typename T, int R>
 struct TileGeom {
@@ -582,7 +588,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
   const int cb = swz(cr % G::TY), cc = cr / G::TY;
   const T* sPc = sP + ((cc + G::NG) * G::BY + (cb + G::NG)) * G::BX + (ca + G::HX);
   const T* sMc = sM + ((cc + 1) * G::MY + (cb + 1)) * G::BX + (ca + G::HX);
-  int fail = 0, reset = 0, pfl = 0, it = 0;
+  int fail = 0, reset = 0, pfl = 0, it = 0, nstall = 0;
   unsigned parity = 0;
 
 #pragma unroll 1
@@ -696,8 +702,9 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       if (!cleaning_<FAST>(par2)) w[8] = 0;
       if (evar_<FAST>(par2)) w[4] = energy_to_tau(w, m2);
       T2 qn[NV];
-      int its = 0;
-      const int fl = con2prim(w, m2, gi, par2, Zg, qn, its);
+      int its = 0, stl = 0;
+      const int fl = con2prim(w, m2, gi, par2, Zg, qn, its, stl);
+      nstall += stl;
       it = its > it ? its : it;
       bool rs = fl != 0;
       if (!rs && qn[RHO] < par2.rho_thr) rs = true;
@@ -728,14 +735,16 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       store_prims_with_images(L, Pout, ci, cj, ck, qs);
     }
   }
-  // warp-level reduction of the counters: [0] c2p_fail, [1] atm_reset, [2] p_floor, [3] max iterations
+  // warp-level reduction of the counters: [0] c2p_fail, [1] atm_reset, [2] p_floor, [3] max iterations,
+  // [4] recoveries ended by the fp32 round-off rule
   const unsigned full = 0xffffffffu;
   const int nf = __reduce_add_sync(full, fail), nr = __reduce_add_sync(full, reset), np = __reduce_add_sync(full, pfl);
-  const int mi = __reduce_max_sync(full, it);
+  const int mi = __reduce_max_sync(full, it), ns = __reduce_add_sync(full, nstall);
   if (lane == 0) {
     if (nf) atomicAdd(counters + 0, (unsigned long long)nf);
     if (nr) atomicAdd(counters + 1, (unsigned long long)nr);
     if (np) atomicAdd(counters + 2, (unsigned long long)np);
+    if (ns) atomicAdd(counters + 4, (unsigned long long)ns);
     if ((unsigned long long)mi > counters[3]) atomicMax(counters + 3, (unsigned long long)mi);
   }
 }

@@ -184,7 +184,7 @@ class SlabGroup:
 
 
 SUM_KEYS = ("sumD", "sumSx", "sumSy", "sumSz", "sumTau", "sumBx", "sumBy", "sumBz", "sumPsi",
-            "c2p_fail", "atm_reset", "p_floor")
+            "c2p_fail", "atm_reset", "p_floor", "c2p_stalled")
 MAX_KEYS = ("divB_max", "max_speed_over_dx", "c2p_maxit_seen")
 
 
@@ -237,7 +237,7 @@ class DistSlabHorizon:
         out = {k: float(v) for k, v in zip(SUM_KEYS, sums[:len(SUM_KEYS)].tolist())}
         out.update({k: float(v) for k, v in zip(MAX_KEYS, maxs.tolist())})
         out["divB_L1"] = float(sums[-2] / sums[-1])
-        for k in ("c2p_fail", "atm_reset", "p_floor", "c2p_maxit_seen"):
+        for k in ("c2p_fail", "atm_reset", "p_floor", "c2p_stalled", "c2p_maxit_seen"):
             out[k] = int(round(out[k]))
         return out
 

@@ -36,7 +36,7 @@ def test_split_and_boundary_codes():
 
 def test_diagnostics_fold():
     d1 = dict(sumD=1.0, sumSx=0.0, sumSy=0.0, sumSz=0.0, sumTau=2.0, sumBx=0.0, sumBy=0.0, sumBz=0.0, sumPsi=0.0,
-              c2p_fail=1, atm_reset=2, p_floor=0, divB_max=3.0, max_speed_over_dx=5.0, c2p_maxit_seen=4, divB_L1=1.0)
+              c2p_fail=1, atm_reset=2, p_floor=0, c2p_stalled=3, divB_max=3.0, max_speed_over_dx=5.0, c2p_maxit_seen=4, divB_L1=1.0)
     d2 = dict(d1, sumD=2.0, divB_max=1.0, max_speed_over_dx=7.0, divB_L1=4.0, c2p_fail=0)
     out = slab.combine_diagnostics([d1, d2], [100, 300])
     assert out["sumD"] == 3.0 and out["sumTau"] == 4.0 and out["c2p_fail"] == 1 and out["atm_reset"] == 4
