@@ -365,44 +365,104 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
   if (!par.cleaning) Phi[8] = 0;
 }
 
-// ---- a6 from the staged metric: centred differences, fluid and cleaning sources at a cell ----------
-// sMc: staged metric at the cell (field 0).  Same arithmetic as add_sources (hz_kernels.cuh).
+// ---- a6 at one cell: geometric and cleaning sources in the 3+1 form of the stress-energy contraction,
+// accumulated ONE AXIS AT A TIME.  With A^{ik} = (rho h + b^2) ut^i ut^k + p* gamma^{ik} - Bt^i Bt^k
+// (ut^i = W v^i the stored primitive, Bt^i = B^i / W + (B.v) ut^i), S_i, S^i the momentum density and
+// E = tau + D, the contraction (1/2) T^{mu nu} d_j g_{mu nu} and the stationary-metric identity of O6 become
+//   alpha Sigma(S_j) = alpha (1/2) A^{ik} d_j gamma_ik + S_i d_j beta^i - E d_j alpha
+//   alpha Sigma(tau) = beta^j (1/2) A^{ik} d_j gamma_ik + A^{jl} gamma_lk d_j beta^k - S^j d_j alpha
+// (T^{00} beta^i beta^k + 2 T^{0(i} beta^{k)} + T^{ik} = A^{ik}, alpha T^0_i = S_i, alpha^2 T^{00} = E: the same
+// numbers as fluid_source up to rounding, with half the arithmetic and no division by the lapse).  Every term is
+// a sum over the axis of differentiation, so the ten metric differences of one axis are formed, used and dropped
+// before the next axis is touched.
+// sPc / sMc: staged primitives / metric at the cell; sRc: its slot in sR; clc: its entry of the static cleaning
+// coefficients of k_clean_static (field stride fs); gmask: bit j set = axis j active.
 template <typename T, int R, int FAST>
-__device__ __forceinline__ void add_sources_staged(const Layout& L, const T* __restrict__ sMc, const T* m, const T* q,
-                                                   const Par<T>& par, const T* gi, T sq, const T* cl4, T* Rs) {
+__device__ __forceinline__ void source_cell(const T* __restrict__ sPc, const T* __restrict__ sMc, T* __restrict__ sRc,
+                                           const T* __restrict__ clc, long long fs, int gmask, T gg1, T kappa, T ih0, T ih1,
+                                           T ih2, int cleaning, int evar) {
   using G = TileGeom<T, R>;
-  T dm[3][NM];
-  // cl4 = (sum_j d_j(alpha sqrt(gamma) gamma^{kj}), k = x y z; sum_j d_j(sqrt(gamma) beta^j)): the metric does
-  // not change in time, so these four coefficients of the cleaning sources are computed once (k_clean_static)
+  T q[NV], m[NM];
 #pragma unroll
-  for (int d = 0; d < 3; d++) {
-    if (L.g[d] == 0) {
+  for (int v = 0; v < NV; v++) q[v] = sPc[v * G::PFS];
 #pragma unroll
-      for (int a = 0; a < NM; a++) dm[d][a] = 0;
-      continue;
-    }
-    const int s = d == 0 ? 1 : (d == 1 ? G::BX : G::BX * G::MY);
-    const T i2h = T(0.5) * par.ih[d];
-    T mp[NM], mm[NM];
+  for (int v = 0; v < NM; v++) m[v] = sMc[v * G::MFS];
+  const T* g = m + GXX;
+  T cf[6];
+  const T det = cofactors(g, cf);
+  const T sq = sqrt_(det);
+  const T idet = rcp_(det);
+  // O1 at the cell
+  T utl[3], Bl[3];
+  lower(g, q + UX, utl);
+  lower(g, q + BX, Bl);
+  const T ut2 = dot3(q + UX, utl);
+  const T W2 = 1 + ut2;
+  const T iW = rsqrt_(W2);
+  const T iW2 = iW * iW;
+  const T rhoh = q[RHO] + gg1 * q[PR];
+  const T B2 = dot3(q + BX, Bl);
+  const T Bv = dot3(q + BX, utl) * iW;         // B.v
+  const T b2 = B2 * iW2 + Bv * Bv;
+  const T pstar = q[PR] + b2 * T(0.5);
+  const T hb = rhoh + b2;
+  const T Z = rhoh * W2;
+  const T ZB = (Z + B2) * iW;                  // (Z + B^2) / W : S = ZB ut - Bv B with either index position
+  const T E = Z - q[PR] + (B2 * (1 + ut2 * iW2) - Bv * Bv) * T(0.5);   // tau + D
+  T Bt[3], Sl[3], Su[3];
 #pragma unroll
-    for (int a = 0; a < NM; a++) { mp[a] = sMc[a * G::MFS + s]; mm[a] = sMc[a * G::MFS - s]; }
-#pragma unroll
-    for (int a = 0; a < NM; a++) dm[d][a] = (mp[a] - mm[a]) * i2h;
+  for (int i = 0; i < 3; i++) {
+    Bt[i] = q[BX + i] * iW + Bv * q[UX + i];
+    Sl[i] = ZB * utl[i] - Bv * Bl[i];
+    Su[i] = ZB * q[UX + i] - Bv * q[BX + i];
   }
-  fluid_source(q, m, dm, par, gi, sq, Rs);
-  if (cleaning_<FAST>(par)) {  // cleaning sources (R14), not multiplied by alpha
+  const T pg = pstar * idet;                   // p* gamma^{ik} = p* cof_ik / det
+  T A[6];                                      // packed (xx xy xz yy yz zz)
 #pragma unroll
-    for (int k = 0; k < 3; k++) {
-      const T adv = q[BX] * dm[0][BEX + k] + q[BY] * dm[1][BEX + k] + q[BZ] * dm[2][BEX + k];
-      Rs[5 + k] += -sq * adv + q[PSI] * cl4[k];
-    }
-    const T Bda = q[BX] * dm[0][AL] + q[BY] * dm[1][AL] + q[BZ] * dm[2][AL];
-    Rs[8] += sq * Bda - q[PSI] * cl4[3] - m[AL] * par.kappa * sq * q[PSI];
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int k = i; k < 3; k++) A[sym(i, k)] = hb * q[UX + i] * q[UX + k] + pg * cf[sym(i, k)] - Bt[i] * Bt[k];
+  const T al = m[AL];
+  const T* be = m + BEX;
+  T Rs[NV];
+  T sT = 0, adv[3] = {0, 0, 0}, Bda = 0;
+  Rs[1] = Rs[2] = Rs[3] = 0;
+#pragma unroll
+  for (int j = 0; j < 3; j++) {
+    if (((gmask >> j) & 1) == 0) continue;
+    asm volatile("" ::: "memory");   // one axis at a time: keeps the staged loads of the next axis behind this one
+    const int st = j == 0 ? 1 : (j == 1 ? G::BX : G::BX * G::MY);
+    const T h = T(0.5) * (j == 0 ? ih0 : (j == 1 ? ih1 : ih2));
+    T d[NM];   // twice the centred difference times the spacing: the factor h = 1 / (2 dx) is applied to the sums
+#pragma unroll
+    for (int v = 0; v < NM; v++) d[v] = sMc[v * G::MFS + st] - sMc[v * G::MFS - st];
+    const T* dg = d + GXX;
+    const T Gj = T(0.5) * (A[0] * dg[0] + A[3] * dg[3] + A[5] * dg[5]) + A[1] * dg[1] + A[2] * dg[2] + A[4] * dg[4];
+    Rs[1 + j] = (sq * h) * (al * Gj + dot3(Sl, d + BEX) - E * d[AL]);
+    // row j of A lowered with gamma: A^{jl} gamma_lk
+    const T row[3] = {A[sym(j, 0)], A[sym(j, 1)], A[sym(j, 2)]};
+    T rl[3];
+    lower(g, row, rl);
+    sT += h * (be[j] * Gj + dot3(rl, d + BEX) - Su[j] * d[AL]);
+    const T Bh = q[BX + j] * h;
+#pragma unroll
+    for (int k = 0; k < 3; k++) adv[k] += Bh * d[BEX + k];
+    Bda += Bh * d[AL];
+  }
+  Rs[4] = sq * sT;
+  // cleaning sources (R14), not multiplied by alpha; clc: the static coefficients of k_clean_static
+  if (FAST || cleaning) {
+    const T psi = q[PSI];
+#pragma unroll
+    for (int k = 0; k < 3; k++) Rs[5 + k] = -sq * adv[k] + psi * clc[k * fs];
+    Rs[8] = sq * Bda - psi * clc[3 * fs] - m[AL] * kappa * sq * psi;
   } else {
-    Rs[8] = 0;
+    Rs[5] = Rs[6] = Rs[7] = Rs[8] = 0;
   }
+  if (!FAST && evar) Rs[4] = 0;  // R1b: no source on a fixed metric
+#pragma unroll
+  for (int v = 1; v < NV; v++) sRc[(v - 1) * G::NC] = Rs[v];
 }
-
 // ---- a9 fused: store the primitives of cell (i,j,k) and of every ghost cell that mirrors it --------
 // Ghost images of interior coordinate c along axis d (O9): periodic -- c + n if c < ng, c - n if
 // c >= n - ng; zero gradient -- the edge cell fills the ng layers beyond it; external sides get none.
@@ -513,30 +573,9 @@ __device__ __forceinline__ void source_task(const Layout& L, const Par<T>& par, 
   if (x0 + a >= L.n[0] || y0 + b >= L.n[1] || z0 + c >= L.n[2]) return;
   const T* sPc = sP + ((c + G::NG) * G::BY + (b + G::NG)) * G::BX + (a + G::HX);
   const T* sMc = sM + ((c + 1) * G::MY + (b + 1)) * G::BX + (a + G::HX);
-  T q[NV], m[NM];
-#pragma unroll
-  for (int v = 0; v < NV; v++) q[v] = sPc[v * G::PFS];
-#pragma unroll
-  for (int v = 0; v < NM; v++) m[v] = sMc[v * G::MFS];
-  T cf[6], gi[6];
-  const T det = cofactors(m + GXX, cf);
-  const T sq = sqrt_(det);
-  const T idet = rcp_(det);
-#pragma unroll
-  for (int a6 = 0; a6 < 6; a6++) gi[a6] = cf[a6] * idet;
-  T Rs[NV];
-#pragma unroll
-  for (int v = 0; v < NV; v++) Rs[v] = 0;
-  T cl4[4] = {0, 0, 0, 0};
-  if (cleaning_<FAST>(par)) {
-    const long long id = L.idx(x0 + a, y0 + b, z0 + c);
-#pragma unroll
-    for (int v = 0; v < 4; v++) cl4[v] = cln[v * L.fs + id];
-  }
-  add_sources_staged<T, R, FAST>(L, sMc, m, q, par, gi, sq, cl4, Rs);
-  if (evar_<FAST>(par)) Rs[4] = 0;  // R1b: no source on a fixed metric
-#pragma unroll
-  for (int v = 1; v < NV; v++) sR[(v - 1) * G::NC + cell] = Rs[v];
+  const int gmask = (L.g[0] ? 1 : 0) | (L.g[1] ? 2 : 0) | (L.g[2] ? 4 : 0);
+  source_cell<T, R, FAST>(sPc, sMc, sR + cell, cln + L.idx(x0 + a, y0 + b, z0 + c), L.fs, gmask, par.gg1, par.kappa,
+                          par.ih[0], par.ih[1], par.ih[2], par.cleaning, par.energy_var);
 }
 
 // One thread: the two TMA boxes of `tile` (primitives, metric), completion on `bar`.
