@@ -391,101 +391,6 @@ __device__ __forceinline__ void flux_speeds(const T* q, const T* m, const T* gid
   }
 }
 
-// ---- O5: HLLE flux through one face, Phi = sqrt(gamma_f) * Fhat --------------
-// qL, qR: reconstructed states (floored here); mf: face metric (mean of the two cells, R8).
-template <typename T, int D>
-__device__ __forceinline__ void hlle_face(T* qL, T* qR, const T* mf, const Par<T>& par, T* Phi) {
-  qL[RHO] = max_(qL[RHO], par.rho_atm); qL[PR] = max_(qL[PR], par.p_atm);
-  qR[RHO] = max_(qR[RHO], par.rho_atm); qR[PR] = max_(qR[PR], par.p_atm);
-  T c[6];
-  const T det = cofactors(mf + GXX, c);
-  const T sq = sqrt_(det);
-  const T idet = rcp_(det);
-  T gid[3];
-#pragma unroll
-  for (int k = 0; k < 3; k++) gid[k] = c[sym(k, D)] * idet;
-  T UL[NV], FL[NV], UR[NV], FR[NV], lmL, lpL, lmR, lpR;
-  flux_speeds<T, D>(qL, mf, gid, par, UL, FL, lmL, lpL);
-  flux_speeds<T, D>(qR, mf, gid, par, UR, FR, lmR, lpR);
-  const T lp = max_(T(0), max_(lpL, lpR));
-  const T lm = min_(T(0), min_(lmL, lmR));
-  const T w = lp - lm;
-  if (w > T(1e-30)) {
-    const T sw = div_(sq, w), ll = lp * lm;
-#pragma unroll
-    for (int q = 0; q < NV; q++) Phi[q] = sw * (lp * FL[q] - lm * FR[q] + ll * (UR[q] - UL[q]));
-  } else {
-#pragma unroll
-    for (int q = 0; q < NV; q++) Phi[q] = sq * T(0.5) * (FL[q] + FR[q]);
-  }
-  if (!par.cleaning) Phi[8] = 0;
-}
-
-// ---- O6: geometric sources at a cell (eq. 2, the Gamma term) ------------------------
-// dm[j][c] = d_j met10[c] (zero rows for inactive axes).  Adds alpha*sqrt(gamma)*Sigma to R[1..4].
-template <typename T>
-__device__ __forceinline__ void fluid_source(const T* q, const T* m, const T (*dm)[NM], const Par<T>& par,
-                                             const T* gi /*6*/, T sq, T* R) {
-  State<T> s;
-  eval_state(q, m, par, s);
-  const T al = m[AL];
-  const T ial = rcp_(al), ial2 = ial * ial;
-  const T* be = m + BEX;
-  T u[4], b[4];
-  u[0] = s.W * ial;
-  b[0] = s.W * s.Bv * ial;
-#pragma unroll
-  for (int i = 0; i < 3; i++) {
-    T vti = s.v[i] - be[i] * ial;
-    u[1 + i] = s.W * vti;
-    b[1 + i] = q[BX + i] * s.iW + s.W * s.Bv * vti;
-  }
-  const T hb = s.rhoh + s.b2;
-  // T^{mu nu} = (rho h + b^2) u u + p* g^{mu nu} - b b
-  const T T00 = hb * u[0] * u[0] - s.pstar * ial2 - b[0] * b[0];
-  T T0[3], Tij[6];
-#pragma unroll
-  for (int i = 0; i < 3; i++) T0[i] = hb * u[0] * u[1 + i] + s.pstar * be[i] * ial2 - b[0] * b[1 + i];
-#pragma unroll
-  for (int i = 0; i < 3; i++)
-#pragma unroll
-    for (int k = i; k < 3; k++)
-      Tij[sym(i, k)] = hb * u[1 + i] * u[1 + k] + s.pstar * (gi[sym(i, k)] - be[i] * be[k] * ial2) - b[1 + i] * b[1 + k];
-  T bl[3];
-  lower(m + GXX, be, bl);
-  T T0l[3], gT0[3];  // T^0_i = beta_i T^{00} + gamma_ik T^{0k}
-  lower(m + GXX, T0, gT0);
-#pragma unroll
-  for (int i = 0; i < 3; i++) T0l[i] = bl[i] * T00 + gT0[i];
-  T SigS[3];
-#pragma unroll
-  for (int j = 0; j < 3; j++) {
-    const T* dg = dm[j] + GXX;
-    T w[3];
-    lower(dg, be, w);  // d_j gamma_ik beta^k
-    T bbdg = dot3(be, w);
-    T t0bdg = dot3(T0, w);
-    T t0db = dot3(T0l, dm[j] + BEX);
-    T tdg = Tij[0] * dg[0] + Tij[3] * dg[3] + Tij[5] * dg[5] + 2 * (Tij[1] * dg[1] + Tij[2] * dg[2] + Tij[4] * dg[4]);
-    SigS[j] = T00 * (bbdg * T(0.5) - al * dm[j][AL]) + t0bdg + t0db + tdg * T(0.5);
-  }
-  // T^i_j d_i beta^j with T^i_j = beta_j T^{i0} + gamma_jk T^{ik}
-  T Tdb = 0;
-#pragma unroll
-  for (int i = 0; i < 3; i++) {
-    T row[3] = {Tij[sym(i, 0)], Tij[sym(i, 1)], Tij[sym(i, 2)]};
-    T rl[3];
-    lower(m + GXX, row, rl);
-#pragma unroll
-    for (int j = 0; j < 3; j++) Tdb += (bl[j] * T0[i] + rl[j]) * dm[i][BEX + j];
-  }
-  T T0da = T0[0] * dm[0][AL] + T0[1] * dm[1][AL] + T0[2] * dm[2][AL];
-  T SigTau = (dot3(be, SigS) + Tdb) * ial - T0da;
-  const T f = al * sq;
-  R[1] += f * SigS[0]; R[2] += f * SigS[1]; R[3] += f * SigS[2];
-  R[4] += f * SigTau;
-}
-
 // ---- O8: primitive recovery, Newton-Raphson on Z = rho h W^2 (R10, R11) -------
 template <typename T>
 struct C2P { T D, S2, B2, SB, E; };

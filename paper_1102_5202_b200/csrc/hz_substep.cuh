@@ -303,8 +303,8 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
         qL[q] = e.v.x;
         qR[q] = e.v.y;
       } else {
-        qL[q] = q0 + T(0.5) * mc_slope(qm, q0, q1);
-        qR[q] = q1 - T(0.5) * mc_slope(q0, q1, q2);
+        qL[q] = q0 + mc_half_slope(qm, q0, q1);
+        qR[q] = q1 - mc_half_slope(q0, q1, q2);
       }
     }
   }
