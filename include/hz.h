@@ -102,10 +102,14 @@ int hz_default_params(hz_params* p);
  * two primitive sets, conserved, conserved at the step start, staging and reduction scratch).
  * HZ_EINVAL on a bad grid or dtype.  Needs no GPU. */
 int hz_state_bytes(const hz_grid* grid, int dtype, size_t* bytes);
+/* The same for the layout hz_create builds with `params` (NULL = defaults): 2 ghost layers with the MC
+ * reconstruction, 3 with PPM; hz_state_bytes above is the larger of the two, enough for either. */
+int hz_state_bytes_for(const hz_grid* grid, int dtype, const hz_params* params, size_t* bytes);
 
 /* Create a context.  `device_buffer` is either NULL (the library allocates hz_state_bytes with
  * cudaMalloc and frees it in hz_destroy) or a caller-owned DEVICE buffer of at least hz_state_bytes
- * bytes, 256-byte aligned (e.g. a torch.uint8 tensor's data_ptr()), which must outlive the context.
+ * bytes (hz_state_bytes_for(.., params, ..) suffices), 256-byte aligned (e.g. a torch.uint8 tensor's data_ptr()), which
+ * must outlive the context.
  * `params` may be NULL (defaults).  Errors: HZ_EINVAL (bad grid: n < 1, 1 < n < 2 along an axis,
  * spacing <= 0, unknown bc or dtype, Gamma <= 1, maxit < 1), HZ_ECUDA (no device / CUDA failure),
  * HZ_ENOMEM. */
@@ -131,7 +135,11 @@ int hz_set_primitives(hz_ctx* ctx, const void* prim8);
 /* Advance n full third-order Runge-Kutta steps (= 3n substeps) with the fixed step dt
  * (PAPER.md:128, 238).  Asynchronous.  HZ_ESTATE before metric and primitives are set or in the
  * middle of a step (after hz_substeps with a count not divisible by 3); HZ_EINVAL if dt <= 0, n < 0.
- * Failed primitive recoveries are not errors: the cell is reset to atmosphere and counted. */
+ * Failed primitive recoveries are not errors: the cell is reset to atmosphere and counted.
+ * With n >= 2 the launches of two consecutive steps (six substeps, after which the double buffers are back in
+ * their roles) are captured once into a CUDA graph and replayed n / 2 times, ordered behind and before the
+ * context stream by events; an odd last step and everything hz_substeps does are plain launches.  The results are
+ * the same bit for bit; the environment variable HZ_NO_GRAPH=1 (read at hz_create) turns the replay off. */
 int hz_step(hz_ctx* ctx, double dt, int n);
 /* Advance `nsub` Runge-Kutta substeps, continuing from the current stage.  Asynchronous. */
 int hz_substeps(hz_ctx* ctx, double dt, int nsub);
@@ -155,8 +163,11 @@ int hz_diagnostics(hz_ctx* ctx, hz_diag* out);
  * hz_halo_unpack writes such a buffer into the ghost planes of that side.  A slab's low-side buffer
  * goes to the high-side ghosts of the slab below it and vice versa.  Both are asynchronous on the context
  * stream.  Call order per substep: hz_substeps(dt, 1) on every slab, pack, transfer, unpack; and once after
- * hz_set_metric (metric) and after hz_set_primitives (primitives).  HZ_EINVAL if z is inactive or the
- * buffer is not device memory; HZ_ESTATE before the fields are set. */
+ * hz_set_metric (metric) and after hz_set_primitives (primitives).  The library keeps track: hz_set_metric,
+ * hz_set_primitives and every substep invalidate the ghost planes of the external sides they outdate, and
+ * hz_substeps / hz_step return HZ_ESTATE instead of advancing a slab whose external ghost planes (metric or
+ * primitives) have not been supplied since.  HZ_EINVAL if z is inactive or the buffer is not device memory;
+ * HZ_ESTATE before the fields are set. */
 enum { HZ_HALO_PRIM = 0, HZ_HALO_METRIC = 1 };
 int hz_halo_bytes(const hz_ctx* ctx, int which, size_t* bytes);
 int hz_halo_pack(hz_ctx* ctx, int which, int side, void* device_buf);
@@ -176,7 +187,7 @@ int hz_fma_peak(int dtype, double* tflops);
  * events on the context stream; hz_profile_read synchronises, adds up the elapsed milliseconds and
  * the launch counts per kernel kind (arrays of HZ_NKERNELS entries, kind k named hz_kernel_name(k))
  * and clears the record.  At most 16384 launches are kept between reads; later ones are not timed. */
-enum { HZ_NKERNELS = 4 };
+enum { HZ_NKERNELS = 2 };
 int hz_profile(hz_ctx* ctx, int enable);
 int hz_profile_read(hz_ctx* ctx, double* ms, long long* launches);
 const char* hz_kernel_name(int kind);

@@ -48,8 +48,9 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        path = _build.build()
-        L = C.CDLL(path)
+        # HZO_LIB: another build of the same source, e.g. the sanitizer build (oracle/build.py --sanitize)
+        path = os.environ.get("HZO_LIB") or _build.build()
+        L = C.CDLL(os.path.abspath(path))
         L.hzo_prim2con_point.argtypes = [_dp, _dp, C.c_double, _dp]
         L.hzo_con2prim_point.argtypes = [_dp, _dp, C.POINTER(OracleParams), C.c_double, _dp, C.POINTER(C.c_int)]
         L.hzo_c2p_residual_point.argtypes = [C.c_double, _dp, _dp, C.c_double]

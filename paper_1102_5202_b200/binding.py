@@ -11,11 +11,11 @@ HZ_HALO_PRIM, HZ_HALO_METRIC = 0, 1
 HZ_OK, HZ_EINVAL, HZ_ENOMEM, HZ_ECUDA, HZ_ESTATE = 0, -1, -2, -3, -4
 
 # every symbol include/hz.h declares (tests check the library exports each of them)
-SYMBOLS = ["hz_default_params", "hz_state_bytes", "hz_create", "hz_destroy", "hz_set_stream", "hz_set_metric",
+SYMBOLS = ["hz_default_params", "hz_state_bytes", "hz_state_bytes_for", "hz_create", "hz_destroy", "hz_set_stream", "hz_set_metric",
            "hz_set_primitives", "hz_step", "hz_substeps", "hz_get_primitives", "hz_get_psi", "hz_get_conserved",
            "hz_diagnostics", "hz_halo_bytes", "hz_halo_pack", "hz_halo_unpack", "hz_launch_count", "hz_fma_peak", "hz_profile", "hz_profile_read", "hz_kernel_name",
            "hz_strerror"]
-HZ_NKERNELS = 4
+HZ_NKERNELS = 2
 
 
 class HzGrid(C.Structure):
@@ -79,6 +79,7 @@ def lib():
         vp, ip = C.c_void_p, C.c_int
         L.hz_default_params.argtypes = [C.POINTER(HzParams)]
         L.hz_state_bytes.argtypes = [C.POINTER(HzGrid), ip, C.POINTER(C.c_size_t)]
+        L.hz_state_bytes_for.argtypes = [C.POINTER(HzGrid), ip, C.POINTER(HzParams), C.POINTER(C.c_size_t)]
         L.hz_create.argtypes = [C.POINTER(HzGrid), ip, C.POINTER(HzParams), vp, C.POINTER(vp)]
         L.hz_destroy.argtypes = [vp]
         L.hz_set_stream.argtypes = [vp, vp]
@@ -153,7 +154,8 @@ class Horizon:
                            (C.c_int * 3)(*[int(b) for b in bc]))
         self.params = params if params is not None else HzParams.default()
         nbytes = C.c_size_t(0)
-        _chk(L.hz_state_bytes(C.byref(self.grid), self.dtype, C.byref(nbytes)), "hz_state_bytes")
+        _chk(L.hz_state_bytes_for(C.byref(self.grid), self.dtype, C.byref(self.params), C.byref(nbytes)),
+             "hz_state_bytes_for")
         self.state_bytes = nbytes.value
         self._buf = None
         buf_ptr = None

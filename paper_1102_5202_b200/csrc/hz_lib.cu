@@ -14,6 +14,17 @@
 
 using namespace hz;
 
+// tiles per block of the tile sequence (make_tile_order)
+#ifndef HZ_SBX
+#define HZ_SBX 4
+#endif
+#ifndef HZ_SBY
+#define HZ_SBY 4
+#endif
+#ifndef HZ_SBZ
+#define HZ_SBZ 8
+#endif
+
 namespace {
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -54,7 +65,7 @@ Layout make_layout(const hz_grid& G, int dtype, int ng) {
 
 // Memory plan: offsets (bytes) of every resident array inside the one device buffer.
 struct Plan {
-  size_t met, cln, P[2], U[2], staging, partials, diag_out, counters, err, total;
+  size_t met, cln, P[2], U[2], staging, partials, diag_out, counters, err, order, total;
   int diag_blocks;
 };
 Plan make_plan(const Layout& L, int dtype) {
@@ -76,6 +87,8 @@ Plan make_plan(const Layout& L, int dtype) {
   p.diag_out = take(NDIAG * sizeof(double));
   p.counters = take(8 * sizeof(unsigned long long));
   p.err = take(sizeof(int));
+  // sequence of the tiles of k_substep (one int per tile; 8 x 4 x 4 cells is the smallest tile of any instantiation)
+  p.order = take(sizeof(int) * (size_t)((L.n[0] + 7) / 8) * ((L.n[1] + 3) / 4) * ((L.n[2] + 3) / 4));
   p.total = o;
   return p;
 }
@@ -105,12 +118,19 @@ struct hz_ctx {
   int pcur;   // P[pcur] holds the current primitives
   int stage;  // next Runge-Kutta stage 0, 1, 2
   bool have_metric, have_prim;
+  bool halo_met[2], halo_prim[2];   // external z sides: ghost planes supplied since the field last changed
   int nsm;                  // multiprocessors of the device (grid of the persistent substep kernel)
   CUtensorMap tmP[2], tmM;  // TMA descriptors of the two primitive sets and of the metric (k_substep stage-in)
   long long launches;
   bool prof;                          // per-kernel event timing on (hz_profile)
+  bool use_graph;                     // hz_step replays step pairs as a CUDA graph (HZ_NO_GRAPH=1 turns it off)
   std::vector<cudaEvent_t> ev_pool;   // pairs: [2i] start, [2i+1] stop
   std::vector<int> ev_kind;           // kind of each recorded pair
+  // hz_step(dt, n >= 2): two full Runge-Kutta steps (6 launches, after which the buffer roles repeat) as one graph
+  cudaGraphExec_t gexec;
+  cudaStream_t gstream;               // capture / replay stream (the context stream may be the legacy default one)
+  cudaEvent_t gev[2];
+  double g_dt; int g_cur, g_pcur;     // what the instantiated graph was captured for
 
   template <typename T> T* met() const { return (T*)(base + plan.met); }
   template <typename T> T* cln() const { return (T*)(base + plan.cln); }
@@ -121,6 +141,7 @@ struct hz_ctx {
   double* diag_out() const { return (double*)(base + plan.diag_out); }
   unsigned long long* counters() const { return (unsigned long long*)(base + plan.counters); }
   int* err() const { return (int*)(base + plan.err); }
+  int* order() const { return (int*)(base + plan.order); }
 };
 
 namespace {
@@ -146,7 +167,7 @@ Par<T> make_par(const hz_ctx* c) {
   return p;
 }
 
-enum { K_SUBSTEP = 0, K_GHOST = 1, K_RESERVED2 = 2, K_RESERVED3 = 3 };
+enum { K_SUBSTEP = 0, K_GHOST = 1 };
 constexpr size_t PROF_MAX = 16384;
 
 // Brackets one launch with events when profiling is on.
@@ -189,6 +210,12 @@ int read_err(hz_ctx* c, int* flag) {
   return HZ_OK;
 }
 
+// An external side (slab decomposition) has ghost planes only the caller can supply.
+inline bool side_external(const hz_ctx* c, int side) { return c->L.g[2] != 0 && bc_side(c->L.bc[2], side) == 2; }
+inline bool halos_valid(const hz_ctx* c, const bool* flags) {
+  return (!side_external(c, 0) || flags[0]) && (!side_external(c, 1) || flags[1]);
+}
+
 template <typename T>
 int set_metric_t(hz_ctx* c, const void* alpha, const void* beta3, const void* gamma6) {
   const Layout& L = c->L;
@@ -205,8 +232,12 @@ int set_metric_t(hz_ctx* c, const void* alpha, const void* beta3, const void* ga
   const long long ntot = (long long)L.N[0] * L.N[1] * L.N[2];
   k_fill_ghosts<T><<<nblocks(ntot, 256), 256, 0, c->stream>>>(L, c->met<T>(), NM);
   HZ_LAUNCHED(c);
-  k_clean_static<T><<<nblocks(n, 256), 256, 0, c->stream>>>(L, c->met<T>(), c->cln<T>());
-  HZ_LAUNCHED(c);
+  c->halo_met[0] = c->halo_met[1] = false;
+  c->halo_prim[0] = c->halo_prim[1] = false;
+  if (halos_valid(c, c->halo_met)) {   // (with an external side the coefficients follow the metric's ghost planes)
+    k_clean_static<T><<<nblocks(n, 256), 256, 0, c->stream>>>(L, c->met<T>(), c->cln<T>());
+    HZ_LAUNCHED(c);
+  }
   int flag = 0;
   if ((rc = read_err(c, &flag))) return rc;
   c->have_prim = false;
@@ -237,6 +268,7 @@ int set_prims_t(hz_ctx* c, const void* prim8) {
   HZ_CUDA(cudaMemsetAsync(c->err(), 0, sizeof(int), c->stream));
   HZ_CUDA(cudaMemsetAsync(c->counters(), 0, 8 * sizeof(unsigned long long), c->stream));
   c->cur = 0; c->u0 = 1; c->pcur = 0; c->stage = 0;
+  c->halo_prim[0] = c->halo_prim[1] = false;
   k_pack_prims<T><<<nblocks(n, 128), 128, 0, c->stream>>>(L, make_par<T>(c), p, c->met<T>(), c->P<T>(0), c->U<T>(0),
                                                           c->err());
   HZ_LAUNCHED(c);
@@ -265,14 +297,15 @@ int substep_tr(hz_ctx* c, double dt) {
       k_substep<float, double, R, FAST><<<grid, G::NT, G::SMEM, c->stream>>>(
           c->tmP[c->pcur], c->tmM, L, make_par<float>(c), make_par<double>(c), (const float*)c->cln<T>(),
           (const float*)Uin, (const float*)U0,
-          (float*)Uout, (float*)c->P<T>(1 - c->pcur), st, dt, c->counters(), ntx, nty, (int)ntiles);
+          (float*)Uout, (float*)c->P<T>(1 - c->pcur), st, dt, c->counters(), ntx, nty, (int)ntiles, c->order());
     else
       k_substep<T, T, R, FAST><<<grid, G::NT, G::SMEM, c->stream>>>(c->tmP[c->pcur], c->tmM, L, par, par, c->cln<T>(), Uin, U0, Uout,
                                                             c->P<T>(1 - c->pcur), st, (T)dt, c->counters(), ntx, nty,
-                                                            (int)ntiles);
+                                                            (int)ntiles, c->order());
   }
   HZ_LAUNCHED(c);
   if (st == 0) { c->u0 = c->cur; c->cur = 1 - c->cur; }
+  c->halo_prim[0] = c->halo_prim[1] = false;   // the new primitives have no external ghost planes yet
   c->pcur = 1 - c->pcur;
   c->stage = (st + 1) % 3;
   return HZ_OK;
@@ -310,10 +343,34 @@ int make_tensor_map(const Layout& L, void* base, int nfields, int bx, int by, in
                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? HZ_OK : HZ_ECUDA;
 }
+// The sequence in which the persistent blocks take the tiles.  In plain x-fastest order the tile above a tile (in
+// z) comes nty * ntx tiles later, and by then the planes the two share have left L2: at 256^3 the primitives and the
+// metric were fetched from HBM 3.3 times per substep (profiles/r02_substep.md).  Taking the tiles in blocks of
+// SBX x SBY x SBZ neighbours (about one wave of the 148 SMs) keeps shared halos in L2; only block surfaces are
+// fetched twice.
+template <typename T, int R>
+int make_tile_order(hz_ctx* c) {
+  using G = TileGeom<T, R>;
+  const Layout& L = c->L;
+  const int nt[3] = {(L.n[0] + G::TX - 1) / G::TX, (L.n[1] + G::TY - 1) / G::TY, (L.n[2] + G::TZ - 1) / G::TZ};
+  const int sb[3] = {HZ_SBX, HZ_SBY, HZ_SBZ};
+  std::vector<int> ord;
+  ord.reserve((size_t)nt[0] * nt[1] * nt[2]);
+  for (int Z = 0; Z < nt[2]; Z += sb[2])
+    for (int Y = 0; Y < nt[1]; Y += sb[1])
+      for (int X = 0; X < nt[0]; X += sb[0])
+        for (int z = Z; z < Z + sb[2] && z < nt[2]; z++)
+          for (int y = Y; y < Y + sb[1] && y < nt[1]; y++)
+            for (int x = X; x < X + sb[0] && x < nt[0]; x++) ord.push_back((z * nt[1] + y) * nt[0] + x);
+  HZ_CUDA(cudaMemcpy(c->order(), ord.data(), ord.size() * sizeof(int), cudaMemcpyHostToDevice));
+  return HZ_OK;
+}
+
 template <typename T, int R>
 int make_maps_tr(hz_ctx* c) {
   using G = TileGeom<T, R>;
   int rc;
+  if ((rc = make_tile_order<T, R>(c))) return rc;
   for (int w = 0; w < 2; w++)
     if ((rc = make_tensor_map<T>(c->L, c->P<T>(w), NV, G::BX, G::BY, G::BZ, &c->tmP[w]))) return rc;
   if ((rc = make_tensor_map<T>(c->L, c->met<T>(), NM, G::BX, G::MY, G::MZ, &c->tmM))) return rc;
@@ -404,10 +461,62 @@ int halo_copy_t(hz_ctx* c, int which, int k0, void* buf, int unpack) {
   const unsigned nb = (unsigned)((tot + 255) / 256 < 4736 ? (tot + 255) / 256 : 4736);
   k_halo_copy<T><<<nb, 256, 0, c->stream>>>(c->L, F, nf, k0, (T*)buf, unpack);
   HZ_LAUNCHED(c);
-  if (unpack && which == HZ_HALO_METRIC) {  // new ghost planes of the metric: its static derivatives follow
-    k_clean_static<T><<<nblocks(c->L.ncell(), 256), 256, 0, c->stream>>>(c->L, c->met<T>(), c->cln<T>());
-    HZ_LAUNCHED(c);
+  if (unpack) {
+    const int side = k0 == 0 ? 0 : 1;
+    (which == HZ_HALO_METRIC ? c->halo_met : c->halo_prim)[side] = true;
+    if (which == HZ_HALO_METRIC && halos_valid(c, c->halo_met)) {
+      // every ghost plane of the metric is in place: its static derivatives follow
+      k_clean_static<T><<<nblocks(c->L.ncell(), 256), 256, 0, c->stream>>>(c->L, c->met<T>(), c->cln<T>());
+      HZ_LAUNCHED(c);
+    }
   }
+  return HZ_OK;
+}
+
+// ---- hz_step(dt, n) with n >= 2: the launches of two full steps replayed as one CUDA graph ------------------
+// After two Runge-Kutta steps (six substeps) the double buffers are back in their roles, so one captured graph
+// serves any number of step pairs.  It pays on small grids, where a substep is shorter than a launch (config 1:
+// 400 cells).  Capture runs on an internal stream (the legacy default stream cannot be captured); the replay is
+// ordered behind the context stream and the context stream behind the replay with two events.
+void graph_drop(hz_ctx* c) {
+  if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+}
+int graph_ready(hz_ctx* c, double dt) {
+  if (c->gexec && c->g_dt == dt && c->g_cur == c->cur && c->g_pcur == c->pcur) return HZ_OK;
+  graph_drop(c);
+  if (!c->gstream) {
+    HZ_CUDA(cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking));
+    HZ_CUDA(cudaEventCreateWithFlags(&c->gev[0], cudaEventDisableTiming));
+    HZ_CUDA(cudaEventCreateWithFlags(&c->gev[1], cudaEventDisableTiming));
+  }
+  const int cur = c->cur, u0 = c->u0, pcur = c->pcur, stage = c->stage;
+  const long long launches = c->launches;
+  const bool hp[2] = {c->halo_prim[0], c->halo_prim[1]};
+  cudaStream_t user = c->stream;
+  c->stream = c->gstream;
+  cudaGraph_t g = nullptr;
+  int rc = HZ_OK;
+  if (cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) rc = HZ_ECUDA;
+  for (int s = 0; s < 6 && rc == HZ_OK; s++) rc = c->dtype == HZ_F64 ? substep_t<double>(c, dt) : substep_t<float>(c, dt);
+  if (cudaStreamEndCapture(c->gstream, &g) != cudaSuccess) rc = rc ? rc : HZ_ECUDA;
+  c->stream = user;   // nothing has run: the bookkeeping goes back to where it was
+  c->cur = cur; c->u0 = u0; c->pcur = pcur; c->stage = stage; c->launches = launches;
+  c->halo_prim[0] = hp[0]; c->halo_prim[1] = hp[1];
+  if (rc == HZ_OK && cudaGraphInstantiate(&c->gexec, g, 0) != cudaSuccess) rc = HZ_ECUDA;
+  if (g) cudaGraphDestroy(g);
+  if (rc != HZ_OK) { cudaGetLastError(); graph_drop(c); return rc; }
+  c->g_dt = dt; c->g_cur = cur; c->g_pcur = pcur;
+  return HZ_OK;
+}
+int step_pairs_graph(hz_ctx* c, double dt, int pairs) {
+  int rc = graph_ready(c, dt);
+  if (rc) return rc;
+  HZ_CUDA(cudaEventRecord(c->gev[0], c->stream));
+  HZ_CUDA(cudaStreamWaitEvent(c->gstream, c->gev[0], 0));
+  for (int p = 0; p < pairs; p++) HZ_CUDA(cudaGraphLaunch(c->gexec, c->gstream));
+  HZ_CUDA(cudaEventRecord(c->gev[1], c->gstream));
+  HZ_CUDA(cudaStreamWaitEvent(c->stream, c->gev[1], 0));
+  c->launches += 6LL * pairs;
   return HZ_OK;
 }
 
@@ -430,6 +539,14 @@ int hz_state_bytes(const hz_grid* grid, int dtype, size_t* bytes) {
   if (!grid_ok(grid) || !bytes || (dtype != HZ_F32 && dtype != HZ_F64 && dtype != HZ_F32_F64)) return HZ_EINVAL;
   // the size of the larger layout (3 ghost layers, PPM): enough for either reconstruction
   *bytes = make_plan(make_layout(*grid, dtype, 3), dtype).total;
+  return HZ_OK;
+}
+
+int hz_state_bytes_for(const hz_grid* grid, int dtype, const hz_params* params, size_t* bytes) {
+  if (!bytes || (dtype != HZ_F32 && dtype != HZ_F64 && dtype != HZ_F32_F64)) return HZ_EINVAL;
+  const int ng = params && params->recon == 1 ? 3 : NG;
+  if (!grid_ok(grid, ng)) return HZ_EINVAL;
+  *bytes = make_plan(make_layout(*grid, dtype, ng), dtype).total;   // exactly what hz_create lays out
   return HZ_OK;
 }
 
@@ -470,8 +587,11 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
   }
   c->cur = 0; c->u0 = 1; c->pcur = 0; c->stage = 0;
   c->have_metric = c->have_prim = false;
+  c->halo_met[0] = c->halo_met[1] = c->halo_prim[0] = c->halo_prim[1] = false;
   c->launches = 0;
   c->prof = false;
+  c->gexec = nullptr; c->gstream = nullptr; c->gev[0] = c->gev[1] = nullptr;
+  c->use_graph = getenv("HZ_NO_GRAPH") == nullptr;
   {
     int dev = 0;
     cudaGetDevice(&dev);
@@ -489,6 +609,8 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
 int hz_destroy(hz_ctx* c) {
   if (!c) return HZ_OK;
   cudaStreamSynchronize(c->stream);
+  graph_drop(c);
+  if (c->gstream) { cudaStreamSynchronize(c->gstream); cudaEventDestroy(c->gev[0]); cudaEventDestroy(c->gev[1]); cudaStreamDestroy(c->gstream); }
   for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
   if (c->own && c->base) cudaFree(c->base);
   delete c;
@@ -498,6 +620,7 @@ int hz_destroy(hz_ctx* c) {
 int hz_set_stream(hz_ctx* c, void* cuda_stream) {
   if (!c) return HZ_EINVAL;
   HZ_CUDA(cudaStreamSynchronize(c->stream));
+  if (c->gstream) HZ_CUDA(cudaStreamSynchronize(c->gstream));
   c->stream = (cudaStream_t)cuda_stream;
   return HZ_OK;
 }
@@ -517,6 +640,8 @@ int hz_substeps(hz_ctx* c, double dt, int nsub) {
   if (!c || nsub < 0 || !(dt > 0) || !std::isfinite(dt)) return HZ_EINVAL;
   if (!c->have_metric || !c->have_prim) return HZ_ESTATE;
   for (int s = 0; s < nsub; s++) {
+    // a slab with an external side cannot take a substep on stale or missing ghost planes
+    if (!halos_valid(c, c->halo_met) || !halos_valid(c, c->halo_prim)) return HZ_ESTATE;
     int rc = HZ_DISPATCH(c, substep_t, c, dt);
     if (rc) return rc;
   }
@@ -526,6 +651,13 @@ int hz_substeps(hz_ctx* c, double dt, int nsub) {
 int hz_step(hz_ctx* c, double dt, int n) {
   if (!c || n < 0) return HZ_EINVAL;
   if (c->have_metric && c->have_prim && c->stage != 0) return HZ_ESTATE;
+  // pairs of steps as one graph replay (not while per-launch events are wanted, and not for a slab with an
+  // external side: its ghost planes must be exchanged between substeps)
+  if (n >= 2 && c->use_graph && !c->prof && dt > 0 && std::isfinite(dt) && c->have_metric && c->have_prim &&
+      !side_external(c, 0) && !side_external(c, 1)) {
+    if (step_pairs_graph(c, dt, n / 2) == HZ_OK) n -= 2 * (n / 2);
+    // (a failed capture falls through to plain launches of all n steps)
+  }
   return hz_substeps(c, dt, 3 * n);
 }
 
@@ -637,7 +769,6 @@ const char* hz_kernel_name(int kind) {
   switch (kind) {
     case K_SUBSTEP: return "k_substep";
     case K_GHOST: return "k_fill_ghosts";
-    case K_RESERVED2: case K_RESERVED3: return "-";
     default: return "?";
   }
 }
@@ -648,7 +779,7 @@ const char* hz_strerror(int e) {
     case HZ_EINVAL: return "invalid argument or unphysical input";
     case HZ_ENOMEM: return "out of device memory";
     case HZ_ECUDA: return "CUDA error or no CUDA device";
-    case HZ_ESTATE: return "call out of order (metric/primitives not set, or mid-step)";
+    case HZ_ESTATE: return "call out of order (metric/primitives not set, mid-step, or ghost planes of an external side not supplied)";
     default: return "unknown error";
   }
 }

@@ -19,9 +19,10 @@
 //              this phase runs in fp64 on fp32 data.
 //
 // The face flux is written ONCE, for a sweep along axis 0: a sweep along axis d reads the vector and
-// metric components cyclically rotated by d (and stores the momentum and field fluxes rotated back),
-// which keeps the code a third of the size of three instantiations -- the unfused kernel was bound by
-// instruction-cache misses (profiles/r01_naive.md).
+// metric components cyclically rotated by d (and stores the momentum and field fluxes rotated back).
+// The general mode compiles that body once, with d a run-time value -- the unfused kernel, with six
+// copies of it, was bound by instruction-cache misses (profiles/r01_naive.md); the fast mode (cleaning on),
+// whose body is half the size, is instantiated per axis.
 #pragma once
 #include <cuda.h>  // CUtensorMap (type only; the encoder is fetched through the runtime, see hz_lib.cu)
 
@@ -372,7 +373,7 @@ __device__ __forceinline__ void face_flux_rot(const T* __restrict__ sPc, const T
 //   alpha Sigma(S_j) = alpha (1/2) A^{ik} d_j gamma_ik + S_i d_j beta^i - E d_j alpha
 //   alpha Sigma(tau) = beta^j (1/2) A^{ik} d_j gamma_ik + A^{jl} gamma_lk d_j beta^k - S^j d_j alpha
 // (T^{00} beta^i beta^k + 2 T^{0(i} beta^{k)} + T^{ik} = A^{ik}, alpha T^0_i = S_i, alpha^2 T^{00} = E: the same
-// numbers as fluid_source up to rounding, with half the arithmetic and no division by the lapse).  Every term is
+// numbers as the T^{mu nu} d_j g_{mu nu} contraction up to rounding, with half the arithmetic and no division by the lapse).  Every term is
 // a sum over the axis of differentiation, so the ten metric differences of one axis are formed, used and dropped
 // before the next axis is touched.
 // sPc / sMc: staged primitives / metric at the cell; sRc: its slot in sR; clc: its entry of the static cleaning
@@ -521,13 +522,24 @@ __device__ __forceinline__ int cdiv(int n) {
 
 // ---- the work items of phase 1 ----------------------------------------------------------------------
 // Face item: 32 consecutive faces of one direction -> Phi into sF.
-template <typename T, int R, int FAST>
+template <typename T, int R, int FAST, int DD = -1>
 __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, const T* sP, const T* sM, T* sF, int task,
                                           int lane, int x0, int y0, int z0) {
   using G = TileGeom<T, R>;
-  int d = (task >= G::WX) + (task >= G::WX + G::WY);
-  // keep ONE copy of the face-flux body: hide the value of d so the compiler does not clone it per axis
-  asm volatile("" : "+r"(d));
+  if constexpr (DD < 0 && FAST) {
+    // One copy of the face item per sweep axis where the body is small (the fast mode): the rotated component and
+    // stride selections become immediates (fp32 +10 %, fp64 +1 %).  The general mode keeps ONE copy with a
+    // run-time axis: its body is twice the size, and three of it overflow the instruction cache
+    // (profiles/r01_naive.md).
+    const int dd = (task >= G::WX) + (task >= G::WX + G::WY);
+    if (dd == 0) face_task<T, R, FAST, 0>(L, par, sP, sM, sF, task, lane, x0, y0, z0);
+    else if (dd == 1) face_task<T, R, FAST, 1>(L, par, sP, sM, sF, task, lane, x0, y0, z0);
+    else face_task<T, R, FAST, 2>(L, par, sP, sM, sF, task, lane, x0, y0, z0);
+    return;
+  }
+  int d = DD >= 0 ? DD : (task >= G::WX) + (task >= G::WX + G::WY);
+  // general mode: hide the value of d so the compiler does not clone the body per axis
+  if constexpr (DD < 0) asm volatile("" : "+r"(d));
   const int off = d == 0 ? 0 : (d == 1 ? G::NFX : G::NFX + G::NFY);                 // first face of d in sF
   const int f = (task - (d == 0 ? 0 : (d == 1 ? G::WX : G::WX + G::WY))) * 32 + lane;  // face number within d
   // (no L.g[d]: indexing a kernel parameter with a run-time d makes the compiler copy it to local memory)
@@ -596,7 +608,7 @@ __device__ __forceinline__ void issue_loads(const CUtensorMap* tmP, const CUtens
 // Uin and Uout are the SAME buffer in stages 1 and 2 (no __restrict__ on them): the update is in place, which is
 // safe because a thread reads only its own cell of U, once, before it writes it.
 // tmP / tmM: tensor maps of the current primitives and of the metric as 4D arrays (x, y, z, field).
-// Tiles are numbered x fastest; block b takes tiles b, b + gridDim.x, ...  While a block is in phase 2
+// Tiles are numbered x fastest; block b takes the tiles order[b], order[b + gridDim.x], ...  While a block is in phase 2
 // of one tile, the TMA loads of its next tile are already in flight (the staged boxes are dead by then).
 // T2 is the arithmetic type of phase 2.  T2 = T: pure fp64 or pure fp32.  T = float with
 // T2 = double is the paper's mixed mode: storage, reconstruction and face fluxes in
@@ -606,7 +618,7 @@ __global__ void __launch_bounds__(Tile<T, R>::NT, 1)
 k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmM, Layout L, Par<T> par,
           Par<T2> par2, const T* __restrict__ cln, const T* Uin, const T* __restrict__ U0, T* Uout,
           T* __restrict__ Pout, int stage, T2 dt, unsigned long long* __restrict__ counters, int ntx, int nty,
-          int ntiles) {
+          int ntiles, const int* __restrict__ order) {
   using G = TileGeom<T, R>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sP = reinterpret_cast<T*>(smem_raw + G::OFF_P);  // sP[field][z][y][x], halo 2 (HX in x)
@@ -618,7 +630,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
 
   if (threadIdx.x == 0) mbar_init(bar, 1);
   __syncthreads();
-  if (threadIdx.x == 0 && (int)blockIdx.x < ntiles) issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, blockIdx.x, ntx, nty);
+  if (threadIdx.x == 0 && (int)blockIdx.x < ntiles) issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, order[blockIdx.x], ntx, nty);
 
   // this thread's cell of phase 2 (one cell per thread), tile-local
   const bool has_cell = G::NT == G::NC || (int)threadIdx.x < G::NC;   // warp-uniform
@@ -631,7 +643,10 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
   unsigned parity = 0;
 
 #pragma unroll 1
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, parity ^= 1u) {
+  for (int ti = blockIdx.x; ti < ntiles; ti += gridDim.x, parity ^= 1u) {
+    // order[]: the sequence in which the tiles are taken (hz_lib.cu: blocks of neighbouring tiles, so that the halo
+    // a tile shares with its neighbours is still in L2 when they ask for it); tile numbers are x fastest
+    const int tile = order[ti];
     const int tx = tile % ntx, tr = tile / ntx;
     const int x0 = tx * G::TX, y0 = (tr % nty) * G::TY, z0 = (tr / nty) * G::TZ;
     const int ci = x0 + ca, cj = y0 + cb, ck = z0 + cc;
@@ -675,8 +690,8 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       Zg = ((T2)sPc[RHO * G::PFS] + par2.gg1 * (T2)sPc[PR * G::PFS]) * (1 + dot3(ut, utl));
     }
     __syncthreads();  // all fluxes and sources are in shared memory; nobody reads sP / sM any more
-    if (threadIdx.x == 0 && tile + (int)gridDim.x < ntiles)
-      issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, tile + gridDim.x, ntx, nty);
+    if (threadIdx.x == 0 && ti + (int)gridDim.x < ntiles)
+      issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, order[ti + gridDim.x], ntx, nty);
 
     // ---- phase 2: one cell per thread, arithmetic in T2 ----
     // 2a: right-hand side from the fluxes and sources in shared memory and the Euler stage u + dt L; after the

@@ -4,7 +4,7 @@ The paper's multi-GPU layer is a block decomposition with a ghost-zone exchange 
 pack kernel -> device-to-host -> MPI -> host-to-device -> unpack kernel.  Here the exchange never leaves
 the devices: `hz_halo_pack` -> NCCL send/recv over NVLink (torch.distributed) -> `hz_halo_unpack`, two
 planes of the nine primitives each way per substep (19 MB per side at 256^2 in fp64, ~25 us on NVLink 5
-against a ~7 ms substep, so it is not overlapped).  All arithmetic stays in the C-ABI library; this
+against a ~5 ms substep; everything is ordered on the device, the host never waits).  All arithmetic stays in the C-ABI library; this
 module only splits arrays, moves buffers and orders calls.
 
 Two transports:
@@ -121,6 +121,9 @@ class DistTransport:
             if nb is not None:
                 recvs.append(dist.P2POp(dist.irecv, recv[side], nb, self.group))
         if sends or recvs:
+            # With NCCL, wait() does not block the host: it makes the current stream wait for the transfer, so
+            # the unpack kernels below are ordered behind it on the device and hz_step stays asynchronous.
+            # (gloo, used by the CPU tests, completes the transfer inside wait().)
             for req in dist.batch_isend_irecv(sends + recvs):
                 req.wait()
         for side in (0, 1):
@@ -129,10 +132,18 @@ class DistTransport:
 
 
 class Slab:
-    """One slab: a Horizon context plus its place in the decomposition."""
+    """One slab: a Horizon context plus its place in the decomposition.
 
-    def __init__(self, w, rank, parts, dtype="f64", **kw):
-        n, h, bc, sl = slab_of(w, rank, parts)
+    `w` is the GLOBAL workload, of which this slab keeps its z range -- or, with local=True, already this rank's
+    own planes of a global grid that no process holds as a whole (weak scaling: workloads.kerr_sweep(zslab=...));
+    w.bc then still names the GLOBAL boundary kinds."""
+
+    def __init__(self, w, rank, parts, dtype="f64", local=False, **kw):
+        if local:
+            n, h, sl = tuple(w.n), tuple(w.h), slice(None)
+            bc = (w.bc[0], w.bc[1], slab_bc(w.bc[2], rank, parts))
+        else:
+            n, h, bc, sl = slab_of(w, rank, parts)
         self.rank, self.parts, self.sl = rank, parts, sl
         self.nb = neighbours(w.bc[2], rank, parts)
         self.ncell = n[0] * n[1] * n[2]
@@ -153,11 +164,15 @@ class Slab:
 
 
 class SlabGroup:
-    """R slabs in one process on one GPU, stepped in lockstep (validation of the exchange)."""
+    """R slabs in one process on one GPU, stepped in lockstep (validation of the exchange).
+    `w`: the global workload, or a list of per-slab workloads (local slabs, see Slab)."""
 
     def __init__(self, w, parts, dtype="f64"):
         self.w, self.parts = w, parts
-        self.slabs = [Slab(w, r, parts, dtype) for r in range(parts)]
+        if isinstance(w, (list, tuple)):
+            self.slabs = [Slab(w[r], r, parts, dtype, local=True) for r in range(parts)]
+        else:
+            self.slabs = [Slab(w, r, parts, dtype) for r in range(parts)]
         self.tr = LocalTransport()
         for s in self.slabs:
             s.set_metric()
@@ -199,15 +214,16 @@ def combine_diagnostics(ds, ncells):
 class DistSlabHorizon:
     """This rank's slab of a global workload under torch.distributed (one process per GPU).
 
-    Every rank builds the same seeded global workload and keeps its z range.  `substeps` runs one substep
-    and one halo exchange at a time; `diagnostics` all-reduces the twelve scalars.
+    Every rank builds the same seeded global workload and keeps its z range -- or (local=True) builds only its
+    own planes.  `substeps` runs one substep and one halo exchange at a time; `diagnostics` all-reduces the
+    scalars.
     """
 
-    def __init__(self, w, dtype="f64", group=None, device="cuda"):
+    def __init__(self, w, dtype="f64", group=None, device="cuda", local=False):
         import torch.distributed as dist
         self.rank, self.parts = dist.get_rank(group), dist.get_world_size(group)
         self.group, self.device = group, device
-        self.slab = Slab(w, self.rank, self.parts, dtype)
+        self.slab = Slab(w, self.rank, self.parts, dtype, local=local)
         self.tr = DistTransport(group)
         self.slab.set_metric()
         self.tr.exchange(self.slab, HZ_HALO_METRIC, device)

@@ -56,7 +56,32 @@ def floor_flip_mask(gpu, ora, rho_atm, atm_tol, band=1e-4):
     return flip & (np.abs(other - thr) <= band * thr)
 
 
+def rel_l1_strict(gpu, ora):
+    """SURVEY.md 8(d) as written, without the GROUP_FLOOR reading: rel. L1 = sum|gpu - ora| / sum|ora| per field;
+    a field that is identically zero in the oracle is reported as max|gpu - ora| / max|vector| instead (the
+    survey's bar for it is 1e-12)."""
+    gpu = np.asarray(gpu, dtype=np.float64)
+    ora = np.asarray(ora, dtype=np.float64)
+    out = {}
+    for f, name in enumerate(FIELDS):
+        den = np.abs(ora[f]).sum()
+        if den > 0:
+            out[name] = np.abs(gpu[f] - ora[f]).sum() / den
+        else:
+            grp = range(1, 4) if 1 <= f <= 3 else (range(5, 8) if f >= 5 else range(f, f + 1))
+            vmax = max(np.abs(ora[g]).max() for g in grp)
+            out[name + "(zero field, max abs / max|vector|)"] = np.abs(gpu[f] - ora[f]).max() / vmax if vmax > 0 else 0.0
+    return out
+
+
 def assert_parity(gpu, ora, tol, what="", mask=None):
+    """Asserts the parity bar under the DESIGN.md section 6 reading and PRINTS what the reading and the mask
+    hide: the number of masked cells and the per-field rel. L1 under SURVEY.md 8(d)'s strict rule (computed
+    over all cells, masked ones included)."""
+    nmask = 0 if mask is None else int(np.count_nonzero(mask))
+    strict = rel_l1_strict(gpu, ora)
+    print(f"[parity] {what}: masked cells {nmask} of {np.asarray(ora)[0].size}; strict rel L1 (no floor, no mask): "
+          + ", ".join(f"{k} {v:.2e}" for k, v in strict.items()))
     if mask is not None:
         gpu = np.where(mask[None], 0.0, np.asarray(gpu, dtype=np.float64))
         ora = np.where(mask[None], 0.0, np.asarray(ora, dtype=np.float64))

@@ -67,6 +67,26 @@ def test_state_bytes_plan(L):
     assert n.value < 40e9
 
 
+def test_state_bytes_for_matches_the_layout_built(L):
+    """hz_state_bytes_for sizes the context for the reconstruction it is created with (the
+    3-ghost PPM size was allocated for every context): MC needs less than the upper bound hz_state_bytes, PPM
+    exactly it; at 256^3 in fp64 the MC context is the 46 + 4 + 10 resident fields DESIGN.md section 4 lists."""
+    nmc, nppm, nup = C.c_size_t(), C.c_size_t(), C.c_size_t()
+    g = grid(256, 256, 256)
+    mc, ppm = B.HzParams.default(), B.HzParams.default(recon=1)
+    assert L.hz_state_bytes_for(C.byref(g), B.HZ_F64, C.byref(mc), C.byref(nmc)) == 0
+    assert L.hz_state_bytes_for(C.byref(g), B.HZ_F64, C.byref(ppm), C.byref(nppm)) == 0
+    assert L.hz_state_bytes(C.byref(g), B.HZ_F64, C.byref(nup)) == 0
+    assert nmc.value < nppm.value == nup.value
+    assert L.hz_state_bytes_for(C.byref(g), B.HZ_F64, None, C.byref(nup)) == 0 and nup.value == nmc.value
+    field = (256 + 4) * (16 + 256 + 16) * (256 + 4) * 8          # padded rows, 2 ghost layers
+    assert 50 * field < nmc.value < 50 * field + 10.5 * 256 ** 3 * 8 + (1 << 22)   # + host staging, scratch
+    # a 2-cell axis is fine with MC, too short for PPM's 3 ghost layers
+    g2 = grid(8, 2, 8)
+    assert L.hz_state_bytes_for(C.byref(g2), B.HZ_F64, C.byref(mc), C.byref(nmc)) == 0
+    assert L.hz_state_bytes_for(C.byref(g2), B.HZ_F64, C.byref(ppm), C.byref(nppm)) == B.HZ_EINVAL
+
+
 @pytest.mark.parametrize("g,dtype", [
     (grid(0, 4, 4), 1), (grid(4, -1, 4), 1), (grid(4, 4, 4, dx=0.0), 1), (grid(4, 4, 4, dx=float("nan")), 1),
     (grid(4, 4, 4, bc=(0, 7, 0)), 1), (grid(4, 4, 4), 5),

@@ -58,3 +58,41 @@ def test_reference_arm_prints_on_rank0_only():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_gpus_flag_starts_one_rank_per_gpu(monkeypatch):
+    """`python bench.py --gpus N` outside torchrun re-executes itself under torch.distributed.run with N ranks on
+    127.0.0.1 (--gpus was ignored by the GPU arm); under torchrun it does not."""
+    sys.path.insert(0, ROOT)
+    import bench
+    calls = []
+    monkeypatch.setattr(bench.subprocess, "call", lambda cmd: calls.append(cmd) or 0)
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    assert bench.main(["--gpus", "4", "--steps", "2", "--warmup", "3", "--shard-weak"]) == 0
+    (cmd,) = calls
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"] and "--nproc-per-node=4" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
+    assert cmd[-7:] == ["--gpus", "4", "--steps", "2", "--warmup", "3", "--shard-weak"]
+    assert os.path.basename(cmd[cmd.index("--master-port") + 2]) == "bench.py"
+
+
+def test_launcher_runs_two_ranks_end_to_end_over_gloo():
+    """The launcher started for real with world_size 2 on CPU: every rank builds only its own slab of the
+    weak-scaling box (PAPER.md:244 shape), the ranks agree on the field scale, rank 0 prints one line."""
+    sys.path.insert(0, ROOT)
+    import bench
+    import workloads as wl
+    stub = os.path.join(ROOT, "tests", "helpers", "rank_stub.py")
+    cmd = bench.launcher_command(["10"], 2, port=29747, script=stub)
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["grid"] == [10, 10, 10] and out["zslab"] == [0, 10] and out["nz_global"] == 20
+    assert out["ms"] >= 20.0                                  # the slower rank's sleep
+    # the global box generated in one piece has the same field maximum as the slabs agreed on
+    import numpy as np
+    g = wl.kerr_sweep(10, zmult=2)
+    assert abs(np.sqrt((g.prim8[5:8] ** 2).sum(axis=0)).max() - out["bmax_euclid"]) <= 1e-12 * out["bmax_euclid"]

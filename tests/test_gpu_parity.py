@@ -248,6 +248,26 @@ def test_bitwise_reproducible():
     assert np.array_equal(outs[0], outs[1])
 
 
+def test_step_graph_replay_equals_plain_launches_bitwise():
+    """hz_step(dt, n >= 2) replays pairs of steps as one CUDA graph (include/hz.h): same kernels, same order, so
+    the state after 5 steps equals 15 plain substeps bit for bit, the launch count is the same, and a second call
+    (buffer roles swapped by the odd step) is right as well."""
+    w = wl.kerr_sweep(20)
+    a, b = horizon(w, "f64"), horizon(w, "f64")
+    n0 = a.launch_count()
+    a.step(w.dt, 5)
+    b.substeps(w.dt, 15)
+    assert a.launch_count() - n0 == 15
+    assert np.array_equal(a.get_primitives(), b.get_primitives())
+    a.step(w.dt, 4)
+    b.substeps(w.dt, 12)
+    assert np.array_equal(a.get_primitives(), b.get_primitives())
+    assert np.array_equal(a.get_conserved(), b.get_conserved())
+    da, db = a.diagnostics(), b.diagnostics()
+    assert da["atm_reset"] == db["atm_reset"] and da["c2p_maxit_seen"] == db["c2p_maxit_seen"]
+    a.close(); b.close()
+
+
 def test_uniform_state_on_constant_curved_metric_is_a_fixed_point():
     n = (20, 12, 9)
     alpha, beta3, gamma6 = wl.constant_metric(n)
@@ -406,6 +426,69 @@ def test_halo_calls_report_errors():
     hz.halo_pack(B.HZ_HALO_PRIM, 1, buf)
     hz.halo_unpack(B.HZ_HALO_PRIM, 1, buf)
     hz.close()
+
+
+def test_external_slab_refuses_to_step_on_stale_ghost_planes():
+    """a slab with an external z side whose ghost planes were never supplied (or not refreshed
+    after a substep or after hz_set_primitives) used to stream zeros or stale planes and return HZ_OK.  Now
+    hz_substeps / hz_step return HZ_ESTATE until both the metric's and the primitives' planes are in place."""
+    import torch
+    from paper_1102_5202_b200 import binding as B
+    from paper_1102_5202_b200.slab import Slab
+    w = wl.kerr_sweep(16)
+    s = Slab(w, 0, 2, "f64")                      # low half: outflow below, EXTERNAL above
+    s.set_metric()
+    s.set_primitives()
+    with pytest.raises(B.HzError) as e:
+        s.hz.substeps(w.dt, 1)                    # no ghost planes at all
+    assert e.value.code == B.HZ_ESTATE
+    mbuf = torch.empty(s.hz.halo_bytes(B.HZ_HALO_METRIC), dtype=torch.uint8, device="cuda")
+    pbuf = torch.empty(s.hz.halo_bytes(B.HZ_HALO_PRIM), dtype=torch.uint8, device="cuda")
+    s.hz.halo_pack(B.HZ_HALO_METRIC, 1, mbuf)     # (any finite planes will do for this test: its own)
+    s.hz.halo_unpack(B.HZ_HALO_METRIC, 1, mbuf)
+    with pytest.raises(B.HzError) as e:
+        s.hz.substeps(w.dt, 1)                    # metric planes supplied, primitives still missing
+    assert e.value.code == B.HZ_ESTATE
+    s.hz.halo_pack(B.HZ_HALO_PRIM, 1, pbuf)
+    s.hz.halo_unpack(B.HZ_HALO_PRIM, 1, pbuf)
+    s.hz.substeps(w.dt, 1)                        # complete: one substep goes through
+    assert np.isfinite(s.hz.get_primitives()).all()
+    with pytest.raises(B.HzError) as e:
+        s.hz.substeps(w.dt, 1)                    # ... and outdates the primitives' planes again
+    assert e.value.code == B.HZ_ESTATE
+    with pytest.raises(B.HzError):
+        s.hz.step(w.dt, 1)
+    s.hz.halo_pack(B.HZ_HALO_PRIM, 1, pbuf)
+    s.hz.halo_unpack(B.HZ_HALO_PRIM, 1, pbuf)
+    s.hz.substeps(w.dt, 1)
+    s.set_primitives()                            # new primitives: their planes are outdated too
+    with pytest.raises(B.HzError) as e:
+        s.hz.substeps(w.dt, 1)
+    assert e.value.code == B.HZ_ESTATE
+    s.hz.close()
+
+
+def test_weak_scaling_slabs_generated_rank_by_rank_reproduce_the_single_box_bitwise():
+    """bench.py --shard-weak (the paper's 120^3 -> 240 x 120^2 shape): every rank generates only its
+    own n^3 slab of the n x n x (n N) Kerr-Schild box.  Three such slabs on one GPU, fed with the rank-by-rank
+    inputs, must give bit for bit what a single context gives on the same inputs put together."""
+    import dataclasses as dc
+    from paper_1102_5202_b200 import SlabGroup
+    n, parts = 14, 3
+    slabs = [wl.kerr_sweep(n, zmult=parts, zslab=(r * n, (r + 1) * n)) for r in range(parts)]
+    g = max(s.extra["bn_max"] for s in slabs)
+    for s in slabs:
+        s.prim8[5:8] *= s.extra["bn_max"] / g
+    cat = lambda f: np.ascontiguousarray(np.concatenate([getattr(s, f) for s in slabs], axis=-3))
+    whole = dc.replace(slabs[0], n=(n, n, n * parts), alpha=cat("alpha"), beta3=cat("beta3"), gamma6=cat("gamma6"),
+                       prim8=cat("prim8"))
+    one = horizon(whole, "f64")
+    grp = SlabGroup(slabs, parts, "f64")
+    one.substeps(whole.dt, 4)
+    grp.substeps(whole.dt, 4)
+    assert np.array_equal(one.get_primitives(), grp.get_primitives())
+    one.close()
+    grp.close()
 
 
 def _paper_sp_dp():

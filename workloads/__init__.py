@@ -326,13 +326,21 @@ def gaussian_field(seed, x, y, z, side=12.0, nmodes=32, nmax=4):
     return out.reshape(len(z), len(y), len(x))
 
 
-def kerr_sweep(nx=128, cfl=0.25, nsteps=34, M=1.0, a=0.9, Bmax=1e-2):
-    n = (nx, nx, nx)
+def kerr_sweep(nx=128, cfl=0.25, nsteps=34, M=1.0, a=0.9, Bmax=1e-2, zmult=1, zslab=None):
+    """BASELINE config 5.  zmult > 1 stacks zmult cubes along z -- the grid is nx x nx x (zmult nx) over
+    z in [-6 zmult, 6 zmult] with the same spacing -- which is the shape of the paper's weak-scaling run
+    (120^3 on one GPU against 240 x 120^2 on two).  zslab = (k0, k1) generates the z planes
+    k0 .. k1-1 of that grid only (one rank's slab; no rank ever holds the whole box); the field is then scaled
+    by the slab's own maximum, which extra['bn_max'] records so that the ranks can agree on the global one."""
+    nz = nx * zmult
+    k0, k1 = (0, nz) if zslab is None else zslab
+    n = (nx, nx, k1 - k0)
     side = 12.0
     x, dx = centres(nx, 4.0, 16.0)
     y, _ = centres(nx, -6.0, 6.0)
+    z = (-6.0 * zmult + (np.arange(k0, k1) + 0.5) * dx)
     ext = lambda c: np.concatenate([[c[0] - dx], c, [c[-1] + dx]])
-    xe, ye, ze = ext(x), ext(y), ext(y)
+    xe, ye, ze = ext(x), ext(y), ext(z)
     Ze, Ye, Xe = np.meshgrid(ze, ye, xe, indexing="ij")
     c = (slice(1, -1),) * 3
     alpha, beta3, gamma6 = kerr_schild(Xe[c], Ye[c], Ze[c], M, a)
@@ -347,7 +355,7 @@ def kerr_sweep(nx=128, cfl=0.25, nsteps=34, M=1.0, a=0.9, Bmax=1e-2):
     prim = np.zeros((8,) + rho.shape)
     prim[0] = rho
     prim[4] = 0.05 * rho
-    w = np.stack([gaussian_field(s, x, y, y, side) for s in (5202, 5203, 5204)])
+    w = np.stack([gaussian_field(s, x, y, z, side) for s in (5202, 5203, 5204)])
     w /= np.sqrt(1.0 + (w * w).sum(axis=0))  # Euclidean |w| < 1, grid independent
     gxx, gxy, gxz, gyy, gyz, gzz = gamma6
     wn = np.sqrt(gxx * w[0] ** 2 + gyy * w[1] ** 2 + gzz * w[2] ** 2 +
@@ -361,7 +369,8 @@ def kerr_sweep(nx=128, cfl=0.25, nsteps=34, M=1.0, a=0.9, Bmax=1e-2):
     prim[5], prim[6], prim[7] = scale * Bx, scale * By, scale * Bz
     params = dict(gamma_ad=4.0 / 3.0, rho_atm=1e-8, p_atm=1e-10, atm_tol=1e-3, cleaning=1, kappa=1.0)
     return Workload("kerr", n, (dx, dx, dx), (BC_OUTFLOW,) * 3, params, np.ascontiguousarray(alpha),
-                    np.ascontiguousarray(beta3), np.ascontiguousarray(gamma6), prim, cfl * dx, nsteps)
+                    np.ascontiguousarray(beta3), np.ascontiguousarray(gamma6), prim, cfl * dx, nsteps,
+                    dict(bn_max=float(Bn.max()), zmult=zmult, zslab=(k0, k1), nz_global=nz))
 
 
 def random_states(seed, count, vmax=0.95, curved=True):
