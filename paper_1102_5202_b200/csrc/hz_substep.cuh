@@ -73,7 +73,7 @@ struct TileGeom {
   static constexpr size_t OFF_M = align128(OFF_P + (size_t)NV * PFS * sizeof(T));
   static constexpr size_t OFF_F = align128(OFF_M + (size_t)NM * MFS * sizeof(T));
   static constexpr size_t OFF_R = align128(OFF_F + (size_t)NV * NF * sizeof(T));
-  static constexpr size_t OFF_BAR = align128(OFF_R + (size_t)(NV - 1) * NC * sizeof(T));  // mbarrier (8 B)
+  static constexpr size_t OFF_BAR = align128(OFF_R + (size_t)(NV - 1) * NC * sizeof(T));  // two mbarriers (8 B each)
   static constexpr size_t SMEM = OFF_BAR + 16;
   static_assert(SMEM <= 227 * 1024, "tile does not fit the 227 KB of shared memory a block may use");
   static constexpr int NFACE_TASKS = WX + WY + WZ, NSRC_TASKS = NC / 32;  // phase-1 work items (one warp each)
@@ -105,6 +105,9 @@ __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
   unsigned done = 0;
@@ -625,10 +628,11 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
   T* sM = reinterpret_cast<T*>(smem_raw + G::OFF_M);  // sM[field][z][y][x], halo 1 (HX in x)
   T* sF = reinterpret_cast<T*>(smem_raw + G::OFF_F);  // sF[q * NF + face]
   T* sR = reinterpret_cast<T*>(smem_raw + G::OFF_R);  // sR[(q-1) * NC + cell]
-  const unsigned bar = smem_addr(smem_raw + G::OFF_BAR);
+  const unsigned bar = smem_addr(smem_raw + G::OFF_BAR);       // the staged boxes of a tile have landed
+  const unsigned bar2 = smem_addr(smem_raw + G::OFF_BAR + 8);  // every warp has read the fluxes and sources of a tile
   const int lane = threadIdx.x & 31;
 
-  if (threadIdx.x == 0) mbar_init(bar, 1);
+  if (threadIdx.x == 0) { mbar_init(bar, 1); mbar_init(bar2, G::NT / 32); }
   __syncthreads();
   if (threadIdx.x == 0 && (int)blockIdx.x < ntiles) issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, order[blockIdx.x], ntx, nty);
 
@@ -653,6 +657,11 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     const bool cell_ok = has_cell && ci < L.n[0] && cj < L.n[1] && ck < L.n[2];
     const long long id = L.idx(ci, cj, ck);
     mbar_wait(bar, parity);
+    // sF / sR may be overwritten once every warp is through phase 2a of the previous tile.  That is an mbarrier the
+    // warps arrive at after 2a and wait on here, not a __syncthreads after 2a: a warp that has its right-hand
+    // sides goes straight on to the Newton iteration (pure arithmetic) while others are still reading fluxes
+    // (bound by shared-memory latency), and the two kinds of work overlap across the warps of the block.
+    if (ti != (int)blockIdx.x) mbar_wait(bar2, parity ^ 1u);
 
     // ---- phase 1: face items, then source items ----
     // Static schedule: the items of a tile cost the same from tile to tile, so warp w takes face items w, w + NW,
@@ -731,7 +740,8 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
 #pragma unroll
       for (int v = 0; v < NV; v++) un[v] = (T2)u[v] + dt * Rh[v];
     }
-    __syncthreads();  // everybody has read sF / sR: the next tile's phase 1 may overwrite them
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar2);   // this warp has read sF / sR (waited on before the next tile's phase 1)
     if (cell_ok) {  // 2b
       // a7: Runge-Kutta stage combine
       if (stage != 0) {
