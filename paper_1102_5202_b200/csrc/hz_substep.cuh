@@ -525,11 +525,14 @@ __device__ __forceinline__ int cdiv(int n) {
 
 // ---- the work items of phase 1 ----------------------------------------------------------------------
 // Face item: 32 consecutive faces of one direction -> Phi into sF.
+#ifndef HZ_AXIS_COPIES_R
+#define HZ_AXIS_COPIES_R 0   // per-axis copies for the MC body only (the PPM body is twice the size)
+#endif
 template <typename T, int R, int FAST, int DD = -1>
 __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, const T* sP, const T* sM, T* sF, int task,
                                           int lane, int x0, int y0, int z0) {
   using G = TileGeom<T, R>;
-  if constexpr (DD < 0 && FAST) {
+  if constexpr (DD < 0 && FAST && R == HZ_AXIS_COPIES_R) {
     // One copy of the face item per sweep axis where the body is small (the fast mode): the rotated component and
     // stride selections become immediates (fp32 +10 %, fp64 +1 %).  The general mode keeps ONE copy with a
     // run-time axis: its body is twice the size, and three of it overflow the instruction cache
