@@ -248,15 +248,19 @@ __device__ __forceinline__ double mc_half_slope(double qm, double q0, double qp)
 }
 __device__ __forceinline__ float mc_half_slope(float qm, float q0, float qp) { return 0.5f * mc_slope(qm, q0, qp); }
 
-// Two MC slopes at once (fp32): differences, doublings and the product packed, min / sign / zero per component.
+// Two MC slopes at once (fp32): differences and doublings packed; per component three min / max and one sign copy.
+// min.xorsign.abs returns min(|a|, |b|) with the sign sign(a) xor sign(b): negative exactly when the two
+// differences have opposite signs, so clamping min(that, |centred|) at zero from below IS the "zero at extrema"
+// rule, and a zero difference gives zero as well; the sign of the result is that of the differences.
+__device__ __forceinline__ float mc_slope_xs(float dm2, float dp2, float c) {
+  float m;
+  asm("min.xorsign.abs.f32 %0, %1, %2;" : "=f"(m) : "f"(dm2), "f"(dp2));
+  return copysignf(fmaxf(fminf(m, fabsf(c)), 0.0f), dp2);
+}
 __device__ __forceinline__ F2 mc_slope(F2 qm, F2 q0, F2 qp) {
   const F2 dm = q0 - qm, dp = qp - q0;
-  const F2 dm2 = dm * 2.0f, dp2 = dp * 2.0f, c = (dm + dp) * 0.5f, pr = dm * dp;
-  float sx = fminf(fminf(fabsf(dm2.v.x), fabsf(dp2.v.x)), fabsf(c.v.x));
-  float sy = fminf(fminf(fabsf(dm2.v.y), fabsf(dp2.v.y)), fabsf(c.v.y));
-  sx = dp.v.x > 0 ? sx : -sx;
-  sy = dp.v.y > 0 ? sy : -sy;
-  return F2(pr.v.x <= 0 ? 0.0f : sx, pr.v.y <= 0 ? 0.0f : sy);
+  const F2 dm2 = dm * 2.0f, dp2 = dp * 2.0f, c = (dm + dp) * 0.5f;
+  return F2(mc_slope_xs(dm2.v.x, dp2.v.x, c.v.x), mc_slope_xs(dm2.v.y, dp2.v.y, c.v.y));
 }
 
 // PPM (O4b / R5b): Colella-Woodward edge values on a uniform mesh, built on the
