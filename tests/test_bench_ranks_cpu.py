@@ -96,3 +96,18 @@ def test_launcher_runs_two_ranks_end_to_end_over_gloo():
     import numpy as np
     g = wl.kerr_sweep(10, zmult=2)
     assert abs(np.sqrt((g.prim8[5:8] ** 2).sum(axis=0)).max() - out["bmax_euclid"]) <= 1e-12 * out["bmax_euclid"]
+
+
+def test_roofline_inputs_belong_to_the_kernels_in_the_tree():
+    """bench.py's DRAM-traffic and flop inputs (profiles/roofline_inputs.json) are ncu measurements of one build of
+    the kernels; the file names that build by a hash of the kernel sources and bench.py flags it stale otherwise
+    (the constants were hard-coded from an earlier build).  The committed file must match."""
+    sys.path.insert(0, ROOT)
+    import bench
+    d = bench.roofline_inputs()
+    assert not d["stale"], (d["kernel_source_sha"], bench.kernel_source_hash())
+    main = d["headline_numerator"]
+    for dt in ("f64", "f32", "f32h"):
+        assert d["flops_per_zone"][main][dt] > 0 and d["dram_bytes_per_zone"][dt] > 0
+    # measured traffic can only exceed the algorithmic byte count (52 words per zone)
+    assert d["dram_bytes_per_zone"]["f64"] >= 52 * 8 and d["dram_bytes_per_zone"]["f32"] >= 52 * 4
