@@ -84,7 +84,8 @@ class LocalTransport:
                     continue
                 # my low ghosts are the high-side planes of the slab below me, and vice versa
                 s.hz.halo_unpack(which, side, bufs[(s.nb[side], 1 - side)])
-        torch.cuda.synchronize()
+        # (no host synchronisation: packs, unpacks and the next substeps are ordered on the stream, and the caching
+        # allocator reuses a freed buffer only behind them on that stream)
 
 
 class DistTransport:
@@ -259,3 +260,42 @@ class DistSlabHorizon:
 
     def close(self):
         self.slab.hz.close()
+
+
+def _time_slabs(n, parts, dtype, steps):
+    """One-GPU measurement of what the slab decomposition itself costs: `parts` slabs of the n^3 Kerr-Schild box as
+    `parts` contexts in one process (pack kernel, device-to-device hand-over, unpack kernel after every substep, the
+    extra ghost planes) against the single context.  It is NOT a multi-GPU measurement: no NCCL, no NVLink."""
+    import json
+    import sys
+    import os
+    import torch
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import workloads as wl
+    w = wl.kerr_sweep(n)
+    out = {}
+    for name, make in (("single", lambda: Horizon.from_workload(w, dtype=dtype)), ("slabs", lambda: SlabGroup(w, parts, dtype))):
+        obj = make()
+        run = (lambda k: obj.substeps(w.dt, 3 * k))
+        run(2)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        run(steps)
+        e1.record()
+        torch.cuda.synchronize()
+        out[name] = w.ncell * 3 * steps / (e0.elapsed_time(e1) * 1e-3)
+        obj.close()
+    out.update(n=n, parts=parts, dtype=dtype, steps=steps, slab_over_single=out["slabs"] / out["single"])
+    print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    import argparse
+    ap = argparse.ArgumentParser(description=_time_slabs.__doc__)
+    ap.add_argument("--n", type=int, default=256)
+    ap.add_argument("--parts", type=int, default=2)
+    ap.add_argument("--dtype", default="f64")
+    ap.add_argument("--steps", type=int, default=5)
+    a = ap.parse_args()
+    _time_slabs(a.n, a.parts, a.dtype, a.steps)
