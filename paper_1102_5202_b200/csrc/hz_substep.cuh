@@ -667,10 +667,28 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     if (ti != (int)blockIdx.x) mbar_wait(bar2, parity ^ 1u);
 
     // ---- phase 1: face items, then source items ----
-    // Static schedule: the items of a tile cost the same from tile to tile, so warp w takes face items w, w + NW,
-    // ...; the source items (about half a face item each) go to the warps that got one face item fewer.  (A
-    // shared-memory work queue with atomics measured 3 % slower: its fetches sat in 6 % of the stall samples.)
-    {
+    // Static schedule: the items of a tile cost the same from tile to tile.  General rule: warp w takes face items
+    // w, w + NW, ...; the source items go to the warps that got one face item fewer.  (A shared-memory work queue
+    // with atomics measured 3 % slower: its fetches sat in 6 % of the stall samples.)
+    if constexpr (sizeof(T) == 8 && G::NFACE_TASKS == 28 && G::NSRC_TASKS == 8 && G::NT == 256) {
+      // fp64 MC tile, 28 + 8 items on 8 warps.  A source item has fewer instructions than a face item but issues them
+      // more slowly (one dependent chain per thread), so the two take about the same time (measured 448 : 494), and
+      // what matters is the mix on each of the four schedulers (warp w runs on scheduler w mod 4): warps 0-3 take
+      // five face items each, warps 4-7 two face items and two source items -- every scheduler then has one warp bound
+      // by the fp64 pipe and one bound by latency: +5 % against the rule below, which balances item counts.  (The
+      // assignment that minimises the longest warp for fixed item durations leaves two warps with source items only:
+      // -16 %; handing a warp consecutive items, all of one sweep axis: -10 %.)
+      const int warp = threadIdx.x >> 5;
+      if (warp < 4) {
+#pragma unroll 1
+        for (int t = warp; t < 20; t += 4) face_task<T, R, FAST>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
+      } else {
+#pragma unroll 1
+        for (int t = 16 + warp; t < 28; t += 4) face_task<T, R, FAST>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
+#pragma unroll 1
+        for (int t = warp - 4; t < 8; t += 4) source_task<T, R, FAST>(L, par, sP, sM, sR, cln, t * 32 + lane, x0, y0, z0);
+      }
+    } else {
       constexpr int NW = G::NT / 32, REM = G::NFACE_TASKS % NW;
       const int warp = threadIdx.x >> 5;
 #pragma unroll 1
