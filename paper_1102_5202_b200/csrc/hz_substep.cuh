@@ -1,6 +1,7 @@
 // hz_substep.cuh -- one Runge-Kutta substep as ONE kernel (rows a1-a9 of DESIGN.md section 2).
 //
-// Blocks are persistent (one per SM) and take tiles of TX x TY x TZ cells round-robin.  Per tile:
+// Blocks are persistent (one per SM) and take tiles of TX x TY x TZ cells in the order of a list (blocks of
+// neighbouring tiles, hz_lib.cu: make_tile_order).  Per tile:
 //   Stage-in : one thread issues two TMA box loads (cp.async.bulk.tensor.4d): the 9 primitives of the
 //              tile with an NG-cell halo (2 for MC, 3 for PPM) and the 10 metric components with a 1-cell
 //              halo (16 bytes of halo along x in both, so every box row starts 16-byte aligned) land in
@@ -10,8 +11,9 @@
 //              direction, every face of the tile exactly once -- reconstruction (MC or PPM), face metric,
 //              left/right states, HLLE; the flux Phi goes to shared memory, never to HBM.
 //              Source items: the geometric and cleaning sources of 32 cells; they need no
-//              flux and fill the gaps the face items leave.
-//   Phase 2  : one cell per thread: flux difference of its six faces + sources from shared memory, Runge-
+//              flux.  One block barrier ends the phase.
+//   Phase 2  : one cell per thread: flux difference of its six faces + sources from shared memory (the flux
+//              buffers are released through an mbarrier, waited on before the next tile's phase 1), Runge-
 //              Kutta stage, Newton-Raphson recovery with the atmosphere floors,
 //              then U and P are written -- P also into the ghost cells that mirror this cell (DESIGN.md
 //              O9), so no boundary kernel runs.  P is double-buffered: neighbours still read the old
@@ -22,7 +24,7 @@
 // metric components cyclically rotated by d (and stores the momentum and field fluxes rotated back).
 // The general mode compiles that body once, with d a run-time value -- the unfused kernel, with six
 // copies of it, was bound by instruction-cache misses (profiles/r01_naive.md); the fast mode (cleaning on),
-// whose body is half the size, is instantiated per axis.
+// whose body is half the size, is instantiated per axis for the MC reconstruction.
 #pragma once
 #include <cuda.h>  // CUtensorMap (type only; the encoder is fetched through the runtime, see hz_lib.cu)
 
