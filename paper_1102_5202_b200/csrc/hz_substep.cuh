@@ -704,9 +704,12 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     // inputs of this thread's cell: conserved state from HBM (latency overlaps the barrier wait), metric and
     // the Newton guess Z = rho h W^2 of the previous primitives from the staged boxes (free for the next
     // tile afterwards)
+    // (in the mixed mode, where phase 2 needs fp64 registers at 128 per thread, the early request would only be
+    // spilled and read back: there U is requested in phase 2a, where it overlaps the flux read)
+    constexpr bool EARLY_U = sizeof(T2) == sizeof(T);
     T u[NV], m[NM];
     T2 Zg = 0;
-    if (cell_ok) {
+    if (EARLY_U && cell_ok) {
 #pragma unroll
       for (int v = 0; v < NV; v++) u[v] = Uin[v * L.fs + id];
     }
@@ -733,6 +736,10 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     T2 un[NV];
     T u0[NV];
     if (cell_ok) {
+      if constexpr (!EARLY_U) {
+#pragma unroll
+        for (int v = 0; v < NV; v++) u[v] = Uin[v * L.fs + id];
+      }
       if (stage != 0) {
 #pragma unroll
         for (int v = 0; v < NV; v++) u0[v] = U0[v * L.fs + id];
