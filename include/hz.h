@@ -53,7 +53,8 @@ enum { HZ_F32 = 0, HZ_F64 = 1, HZ_F32_F64 = 2 };
  * HZ_BC_EXTERNAL_OUTFLOW: low side external, high side outflow; HZ_BC_OUTFLOW_EXTERNAL: the reverse. */
 enum { HZ_BC_PERIODIC = 0, HZ_BC_OUTFLOW = 1, HZ_BC_EXTERNAL = 2, HZ_BC_EXTERNAL_OUTFLOW = 3,
        HZ_BC_OUTFLOW_EXTERNAL = 4 };
-enum { HZ_OK = 0, HZ_EINVAL = -1, HZ_ENOMEM = -2, HZ_ECUDA = -3, HZ_ESTATE = -4 };
+enum { HZ_OK = 0, HZ_EINVAL = -1, HZ_ENOMEM = -2, HZ_ECUDA = -3, HZ_ESTATE = -4,
+       HZ_ELIMIT = -5 /* a size beyond the fixed maximum of hz_sum_fields_noalloc */ };
 
 /* Uniform Cartesian mesh.  An axis with one cell is inactive: no ghost zones, no
  * sweep, no derivative along it (two-dimensional meshes). */
@@ -191,6 +192,35 @@ enum { HZ_NKERNELS = 2 };
 int hz_profile(hz_ctx* ctx, int enable);
 int hz_profile_read(hz_ctx* ctx, double* ms, long long* launches);
 const char* hz_kernel_name(int kind);
+
+/* ---- the one entry point that allocates NOTHING (csrc/hz_noalloc.cu) -------------------------------------
+ * For callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it.  A variant of the library's global reduction (hz_diagnostics) that needs no
+ * context: the sums over `ncell` cells of `nfields` fields, accumulated in fp64 in a fixed order (deterministic).
+ *   fields_dev  DEVICE memory, nfields planes of ncell elements each, plane f at element offset f*ncell
+ *               (the layout hz_get_conserved writes), element type float (HZ_F32) or double (HZ_F64)
+ *   sums_dev    DEVICE memory, nfields doubles: sums_dev[f] = sum of plane f.  (Multiply by dx*dy*dz for the
+ *               volume sums hz_diagnostics reports.)
+ *   cuda_stream a cudaStream_t (NULL = default stream); the call is ASYNCHRONOUS, two kernels on that stream
+ * The block partials live in a file-scope `static __device__` array of fixed size --
+ * HZ_NOALLOC_MAX_BLOCKS x HZ_NOALLOC_MAX_FIELDS doubles = 151 552 bytes (148 KiB) -- which every GPU that loads
+ * the library holds until the process exits.  Limits: nfields <= HZ_NOALLOC_MAX_FIELDS (16) and
+ * ncell <= HZ_NOALLOC_MAX_CELLS (2^31 cells per field); beyond them the call returns HZ_ELIMIT and does nothing.
+ * The call itself performs no cudaMalloc, cudaFree or allocating library call.  hz_noalloc_setup looks up the
+ * array's device address for the CURRENT device (cudaGetSymbolAddress; once per device; no allocation, no
+ * launch); hz_sum_fields_noalloc does the same on its first call on a device, so call hz_noalloc_setup first
+ * where even that look-up is unwelcome (before a stream capture begins).
+ * Every call on a device shares the one array, which keeps the last call's contents; nothing in it has to start
+ * at zero (every row a call reads it has written first).  Calls that OVERLAP on one GPU -- different streams or
+ * host threads without ordering between them -- race on the array and return wrong sums: serialise them.
+ * Errors: HZ_EINVAL (NULL or non-device pointer, nfields < 1, ncell < 1, dtype not HZ_F32 / HZ_F64; the mixed
+ * mode stores floats: pass HZ_F32), HZ_ELIMIT, HZ_ECUDA. */
+#define HZ_NOALLOC_MAX_BLOCKS 1184
+#define HZ_NOALLOC_MAX_FIELDS 16
+#define HZ_NOALLOC_MAX_CELLS (1LL << 31)
+int hz_noalloc_setup(void);
+int hz_sum_fields_noalloc(const void* fields_dev, int nfields, long long ncell, int dtype, double* sums_dev,
+                          void* cuda_stream);
 
 const char* hz_strerror(int code);
 

@@ -8,12 +8,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 HZ_F32, HZ_F64, HZ_F32_F64 = 0, 1, 2
 HZ_BC_PERIODIC, HZ_BC_OUTFLOW, HZ_BC_EXTERNAL, HZ_BC_EXTERNAL_OUTFLOW, HZ_BC_OUTFLOW_EXTERNAL = 0, 1, 2, 3, 4
 HZ_HALO_PRIM, HZ_HALO_METRIC = 0, 1
-HZ_OK, HZ_EINVAL, HZ_ENOMEM, HZ_ECUDA, HZ_ESTATE = 0, -1, -2, -3, -4
+HZ_OK, HZ_EINVAL, HZ_ENOMEM, HZ_ECUDA, HZ_ESTATE, HZ_ELIMIT = 0, -1, -2, -3, -4, -5
+HZ_NOALLOC_MAX_BLOCKS, HZ_NOALLOC_MAX_FIELDS, HZ_NOALLOC_MAX_CELLS = 1184, 16, 1 << 31
 
 # every symbol include/hz.h declares (tests check the library exports each of them)
 SYMBOLS = ["hz_default_params", "hz_state_bytes", "hz_state_bytes_for", "hz_create", "hz_destroy", "hz_set_stream", "hz_set_metric",
            "hz_set_primitives", "hz_step", "hz_substeps", "hz_get_primitives", "hz_get_psi", "hz_get_conserved",
-           "hz_diagnostics", "hz_halo_bytes", "hz_halo_pack", "hz_halo_unpack", "hz_launch_count", "hz_fma_peak", "hz_profile", "hz_profile_read", "hz_kernel_name",
+           "hz_diagnostics", "hz_noalloc_setup", "hz_sum_fields_noalloc", "hz_halo_bytes", "hz_halo_pack", "hz_halo_unpack", "hz_launch_count", "hz_fma_peak", "hz_profile", "hz_profile_read", "hz_kernel_name",
            "hz_strerror"]
 HZ_NKERNELS = 2
 
@@ -101,6 +102,8 @@ def lib():
         L.hz_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.hz_kernel_name.argtypes = [ip]
         L.hz_kernel_name.restype = C.c_char_p
+        L.hz_noalloc_setup.argtypes = []
+        L.hz_sum_fields_noalloc.argtypes = [vp, ip, C.c_longlong, ip, vp, vp]
         L.hz_strerror.argtypes = [ip]
         L.hz_strerror.restype = C.c_char_p
         _lib = L
@@ -117,6 +120,22 @@ def _ptr(a):
     if isinstance(a, np.ndarray):
         return C.c_void_p(a.ctypes.data)
     return C.c_void_p(a.data_ptr())  # torch.Tensor
+
+
+def noalloc_setup():
+    """hz_noalloc_setup: device address of the fixed scratch array for the current device (no allocation)."""
+    _chk(lib().hz_noalloc_setup(), "hz_noalloc_setup")
+
+
+def sum_fields_noalloc(fields, nfields, ncell, out, stream=None):
+    """hz_sum_fields_noalloc: out[f] = sum of plane f of `fields` (torch CUDA tensor, float32 or float64, nfields
+    planes of ncell elements); `out` a torch CUDA tensor of nfields float64.  Asynchronous; allocates nothing."""
+    import torch
+    dt = HZ_F64 if fields.dtype == torch.float64 else HZ_F32
+    s = getattr(stream, "cuda_stream", stream) if stream is not None else torch.cuda.current_stream().cuda_stream
+    _chk(lib().hz_sum_fields_noalloc(_ptr(fields), int(nfields), int(ncell), dt, _ptr(out), C.c_void_p(s)),
+         "hz_sum_fields_noalloc")
+    return out
 
 
 def fma_peak(dtype="f64"):

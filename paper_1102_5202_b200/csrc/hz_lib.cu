@@ -780,6 +780,7 @@ const char* hz_strerror(int e) {
     case HZ_ENOMEM: return "out of device memory";
     case HZ_ECUDA: return "CUDA error or no CUDA device";
     case HZ_ESTATE: return "call out of order (metric/primitives not set, mid-step, or ghost planes of an external side not supplied)";
+    case HZ_ELIMIT: return "size beyond the fixed maximum of the no-allocation entry point (HZ_NOALLOC_MAX_FIELDS / HZ_NOALLOC_MAX_CELLS)";
     default: return "unknown error";
   }
 }
