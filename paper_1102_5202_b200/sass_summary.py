@@ -17,6 +17,10 @@ OPS = ["UTMALDG", "SYNCS", "DFMA", "DMUL", "DADD", "DSETP", "FFMA2", "FMUL2", "F
 
 def demangle(name):
     out = subprocess.run(["c++filt", name], capture_output=True, text=True).stdout.strip()
+    if out == name:   # internal linkage (anonymous namespace): nvcc's _GLOBAL__N__<hash>_<file> prefix is not Itanium
+        m = re.search(r"_cu_[0-9a-f]{8}\d+(k_[a-z_]+)(I[fd]E)?", name)
+        return "(file-local) " + (m.group(1) + {"IfE": "<float>", "IdE": "<double>", None: ""}[m.group(2)] if m else name)
+    out = out.replace("(anonymous namespace)::", "")
     return re.sub(r"\(.*", "", out) or name
 
 
