@@ -650,12 +650,16 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
   const T* sMc = sM + ((cc + 1) * G::MY + (cb + 1)) * G::BX + (ca + G::HX);
   int fail = 0, reset = 0, pfl = 0, it = 0, nstall = 0;
   unsigned parity = 0;
+  int tile_next = (int)blockIdx.x < ntiles ? order[blockIdx.x] : 0;   // tile numbers are fetched one tile ahead
 
 #pragma unroll 1
   for (int ti = blockIdx.x; ti < ntiles; ti += gridDim.x, parity ^= 1u) {
     // order[]: the sequence in which the tiles are taken (hz_lib.cu: blocks of neighbouring tiles, so that the halo
     // a tile shares with its neighbours is still in L2 when they ask for it); tile numbers are x fastest
-    const int tile = order[ti];
+    // (the load of the next number is in flight during phase 1: read at the top of its own iteration it cost 1 % of
+    // the kernel in long-scoreboard stalls)
+    const int tile = tile_next;
+    tile_next = ti + (int)gridDim.x < ntiles ? order[ti + gridDim.x] : 0;
     const int tx = tile % ntx, tr = tile / ntx;
     const int x0 = tx * G::TX, y0 = (tr % nty) * G::TY, z0 = (tr / nty) * G::TZ;
     const int ci = x0 + ca, cj = y0 + cb, ck = z0 + cc;
@@ -726,7 +730,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
     }
     __syncthreads();  // all fluxes and sources are in shared memory; nobody reads sP / sM any more
     if (threadIdx.x == 0 && ti + (int)gridDim.x < ntiles)
-      issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, order[ti + gridDim.x], ntx, nty);
+      issue_loads<T, R>(&tmP, &tmM, L, sP, sM, bar, tile_next, ntx, nty);
 
     // ---- phase 2: one cell per thread, arithmetic in T2 ----
     // 2a: right-hand side from the fluxes and sources in shared memory and the Euler stage u + dt L; after the
