@@ -244,7 +244,9 @@ def time_leg(args, dtype, w, wname, world, rank, local, barrier, sampler, headli
         # PAPER.md:176-178): strong scaling cuts the ONE box, weak scaling gives every rank its own n^3 slab
         from paper_1102_5202_b200 import DistSlabHorizon
         from paper_1102_5202_b200.binding import HZ_HALO_PRIM
-        dsh = DistSlabHorizon(w, dtype=dtype, local=(mode == "weak"))
+        # --exchange fused (default): the neighbours' buffers mapped through CUDA IPC and the exchange done by the
+        # substep kernel's own stores (hz_peer_attach); --exchange nccl: pack kernel, NCCL send/recv, unpack kernel
+        dsh = DistSlabHorizon(w, dtype=dtype, local=(mode == "weak"), fused=(args.exchange == "fused"))
         hz = dsh.slab.hz
         step = lambda: dsh.step(w.dt, 1)
         ncell = dsh.slab.ncell                                   # this rank's zones
@@ -424,8 +426,9 @@ def run_gpu(args):
                "sample": f"{args.ref_n}^3 sub-grid of the same Kerr-Schild sweep, 6 full RK3 steps (18 substeps) after "
                          f"1 warm-up step, fp64, {el:.1f} s; the unoptimised oracle as it stands (plain C++, -O2)"}
 
-    par = {"shard": "z-slabs of the one box, NCCL halo exchange per substep",
-           "weak": "one z-slab per rank, NCCL halo exchange per substep", "replica": "replicas"}[mode]
+    how = ("halo exchange fused into the substep kernel (stores into the IPC-mapped neighbour), one barrier per substep"
+           if args.exchange == "fused" else "NCCL halo exchange per substep")
+    par = {"shard": "z-slabs of the one box, " + how, "weak": "one z-slab per rank, " + how, "replica": "replicas"}[mode]
     line = {
         "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": head["ms_per_step"], "higher_is_better": True,
@@ -476,6 +479,9 @@ def main(argv=None):
     ap.add_argument("--shard", action="store_true",
                     help="with --gpus N > 1: cut the one box into N z-slabs with a halo exchange per substep "
                          "(strong scaling) instead of N independent replicas (weak scaling, the default)")
+    ap.add_argument("--exchange", default="fused", choices=["fused", "nccl"],
+                    help="with --shard / --shard-weak: how the ghost planes travel (fused: peer stores of the substep "
+                         "kernel into the CUDA-IPC-mapped neighbour; nccl: pack kernel, send/recv, unpack kernel)")
     ap.add_argument("--shard-weak", action="store_true",
                     help="with --gpus N > 1: one box of n x n x (n N) cells, one n^3 z-slab per rank, halo exchange "
                          "per substep (weak scaling in the paper's own shape, PAPER.md:244)")

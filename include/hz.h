@@ -174,6 +174,33 @@ int hz_halo_bytes(const hz_ctx* ctx, int which, size_t* bytes);
 int hz_halo_pack(hz_ctx* ctx, int which, int side, void* device_buf);
 int hz_halo_unpack(hz_ctx* ctx, int which, int side, const void* device_buf);
 
+/* The exchange of the primitives FUSED INTO THE SUBSTEP KERNEL (PAPER.md:176-178 exchanges the ghost zones after
+ * every substep with a pack kernel, two copies through the host, MPI and an unpack kernel; PAPER.md:278 names that
+ * synchronisation as the possible limit of the scaling).  Where the neighbour's primitive buffers are addressable
+ * from this device -- another context on the same GPU, a peer GPU of this process (cudaDeviceEnablePeerAccess), or
+ * another process's buffer opened through CUDA IPC -- hz_peer_attach hands them to the context, and from then on
+ * every substep stores the cells within NG planes of that cut, and their x / y ghost images, straight into the
+ * neighbour's ghost planes (over NVLink for a peer GPU) while it writes its own primitives: no pack kernel, no
+ * transfer, no unpack kernel, and hz_halo_pack / hz_halo_unpack of the primitives are needed only once, after
+ * hz_set_primitives.  (The metric's ghost planes are exchanged once with hz_halo_pack / hz_halo_unpack as before.)
+ *   hz_prim_buffers  the DEVICE addresses of this context's two primitive sets (9 fields each, `field_stride`
+ *                    elements apart, padded layout) -- what the neighbour passes to hz_peer_attach.  They are part
+ *                    of the state buffer and live as long as the context.
+ *   hz_peer_attach   side 0 = the neighbour below (low z), 1 = above; peer_P0 / peer_P1 / peer_field_stride: the
+ *                    neighbour's hz_prim_buffers; peer_nz: its interior planes.  The neighbour must have the same
+ *                    nx, ny, dtype, reconstruction and boundary kinds in x and y.  HZ_EINVAL if that side is not
+ *                    external, a pointer is not device memory, or the context does not run the default
+ *                    configuration (cleaning on, energy_var 0: the only kernels compiled with peer stores).
+ *   hz_peer_detach   back to hz_halo_pack / hz_halo_unpack on that side.
+ * Contract: attach MUTUALLY (each of two neighbours attaches the other) and advance the slabs in LOCKSTEP -- every
+ * slab takes substep s before any takes s + 1, and a slab's substep s + 1 is ordered behind its neighbours' substep s
+ * on the device (one stream, an event, or a barrier between processes); the library then regards the ghost planes
+ * of an attached side as supplied after each substep and does not return HZ_ESTATE for them.  Nothing is allocated
+ * and the library keeps only the three pointers; the caller keeps the neighbour's buffers alive. */
+int hz_prim_buffers(hz_ctx* ctx, void** P0, void** P1, long long* field_stride);
+int hz_peer_attach(hz_ctx* ctx, int side, void* peer_P0, void* peer_P1, long long peer_field_stride, int peer_nz);
+int hz_peer_detach(hz_ctx* ctx, int side);
+
 /* Number of kernels this context has launched since hz_create (bench.py's gpu_launches). */
 long long hz_launch_count(const hz_ctx* ctx);
 

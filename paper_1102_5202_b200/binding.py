@@ -14,7 +14,7 @@ HZ_NOALLOC_MAX_BLOCKS, HZ_NOALLOC_MAX_FIELDS, HZ_NOALLOC_MAX_CELLS = 1184, 16, 1
 # every symbol include/hz.h declares (tests check the library exports each of them)
 SYMBOLS = ["hz_default_params", "hz_state_bytes", "hz_state_bytes_for", "hz_create", "hz_destroy", "hz_set_stream", "hz_set_metric",
            "hz_set_primitives", "hz_step", "hz_substeps", "hz_get_primitives", "hz_get_psi", "hz_get_conserved",
-           "hz_diagnostics", "hz_noalloc_setup", "hz_sum_fields_noalloc", "hz_halo_bytes", "hz_halo_pack", "hz_halo_unpack", "hz_launch_count", "hz_fma_peak", "hz_profile", "hz_profile_read", "hz_kernel_name",
+           "hz_diagnostics", "hz_noalloc_setup", "hz_sum_fields_noalloc", "hz_halo_bytes", "hz_halo_pack", "hz_halo_unpack", "hz_prim_buffers", "hz_peer_attach", "hz_peer_detach", "hz_launch_count", "hz_fma_peak", "hz_profile", "hz_profile_read", "hz_kernel_name",
            "hz_strerror"]
 HZ_NKERNELS = 2
 
@@ -95,6 +95,9 @@ def lib():
         L.hz_halo_bytes.argtypes = [vp, ip, C.POINTER(C.c_size_t)]
         L.hz_halo_pack.argtypes = [vp, ip, ip, vp]
         L.hz_halo_unpack.argtypes = [vp, ip, ip, vp]
+        L.hz_prim_buffers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_longlong)]
+        L.hz_peer_attach.argtypes = [vp, ip, vp, vp, C.c_longlong, ip]
+        L.hz_peer_detach.argtypes = [vp, ip]
         L.hz_fma_peak.argtypes = [ip, C.POINTER(C.c_double)]
         L.hz_launch_count.argtypes = [vp]
         L.hz_launch_count.restype = C.c_longlong
@@ -273,6 +276,20 @@ class Horizon:
     def halo_unpack(self, which, side, buf):
         """Device buffer `buf` -> ghost z planes of `side`."""
         _chk(lib().hz_halo_unpack(self._h, int(which), int(side), _ptr(buf)), "hz_halo_unpack")
+
+    def prim_buffers(self):
+        """(P0, P1, field_stride): device addresses of the two primitive sets (what a neighbour's peer_attach takes)."""
+        p0, p1, fs = C.c_void_p(), C.c_void_p(), C.c_longlong(0)
+        _chk(lib().hz_prim_buffers(self._h, C.byref(p0), C.byref(p1), C.byref(fs)), "hz_prim_buffers")
+        return p0.value, p1.value, fs.value
+
+    def peer_attach(self, side, p0, p1, field_stride, nz):
+        """From now on every substep also stores the planes next to `side` into the neighbour's ghost planes."""
+        _chk(lib().hz_peer_attach(self._h, int(side), C.c_void_p(p0), C.c_void_p(p1), int(field_stride), int(nz)),
+             "hz_peer_attach")
+
+    def peer_detach(self, side):
+        _chk(lib().hz_peer_detach(self._h, int(side)), "hz_peer_detach")
 
     def launch_count(self):
         return lib().hz_launch_count(self._h)

@@ -119,6 +119,11 @@ struct hz_ctx {
   int stage;  // next Runge-Kutta stage 0, 1, 2
   bool have_metric, have_prim;
   bool halo_met[2], halo_prim[2];   // external z sides: ghost planes supplied since the field last changed
+  // peer stores (hz_peer_attach): the two primitive sets of the neighbour on each external side, mapped into this
+  // process; its field stride and (side 0) its interior planes.  peer_P[side][0] == nullptr: no neighbour mapped.
+  void* peer_P[2][2];
+  long long peer_fs[2];
+  int peer_nz[2];
   int nsm;                  // multiprocessors of the device (grid of the persistent substep kernel)
   CUtensorMap tmP[2], tmM;  // TMA descriptors of the two primitive sets and of the metric (k_substep stage-in)
   long long launches;
@@ -291,7 +296,32 @@ int substep_tr(hz_ctx* c, double dt) {
   const int ntx = (L.n[0] + G::TX - 1) / G::TX, nty = (L.n[1] + G::TY - 1) / G::TY, ntz = (L.n[2] + G::TZ - 1) / G::TZ;
   const long long ntiles = (long long)ntx * nty * ntz;
   const unsigned grid = (unsigned)(ntiles < c->nsm ? ntiles : c->nsm);  // persistent: one block per SM
-  {
+  if (c->peer_P[0][0] || c->peer_P[1][0]) {
+    // a slab with mapped neighbours: the instantiation that also stores into their ghost planes (fast mode only,
+    // hz_peer_attach refuses the others).  The neighbour's set written in this substep is its P[1 - pcur]: slabs
+    // advance in lockstep, so the roles of their double buffers agree.
+    if constexpr (FAST == 1) {
+      PeerArg<T, 1> pa;
+      for (int s = 0; s < 2; s++) { pa.dst[s] = (T*)c->peer_P[s][1 - c->pcur]; pa.fs[s] = c->peer_fs[s]; }
+      pa.nz0 = c->peer_nz[0];
+      ProfScope ps(c, K_SUBSTEP);
+      if (sizeof(T) == 4 && c->dtype == HZ_F32_F64) {
+        PeerArg<float, 1> pf;
+        for (int s = 0; s < 2; s++) { pf.dst[s] = (float*)c->peer_P[s][1 - c->pcur]; pf.fs[s] = c->peer_fs[s]; }
+        pf.nz0 = c->peer_nz[0];
+        k_substep<float, double, R, FAST, 1><<<grid, G::NT, G::SMEM, c->stream>>>(
+            c->tmP[c->pcur], c->tmM, L, make_par<float>(c), make_par<double>(c), (const float*)c->cln<T>(),
+            (const float*)Uin, (const float*)U0, (float*)Uout, (float*)c->P<T>(1 - c->pcur), st, dt, c->counters(), ntx,
+            nty, (int)ntiles, c->order(), pf);
+      } else {
+        k_substep<T, T, R, FAST, 1><<<grid, G::NT, G::SMEM, c->stream>>>(
+            c->tmP[c->pcur], c->tmM, L, par, par, c->cln<T>(), Uin, U0, Uout, c->P<T>(1 - c->pcur), st, (T)dt,
+            c->counters(), ntx, nty, (int)ntiles, c->order(), pa);
+      }
+    } else {
+      return HZ_ESTATE;
+    }
+  } else {
     ProfScope ps(c, K_SUBSTEP);
     if (sizeof(T) == 4 && c->dtype == HZ_F32_F64)  // fp32 storage and faces, fp64 flux difference / RK / con2prim
       k_substep<float, double, R, FAST><<<grid, G::NT, G::SMEM, c->stream>>>(
@@ -305,7 +335,9 @@ int substep_tr(hz_ctx* c, double dt) {
   }
   HZ_LAUNCHED(c);
   if (st == 0) { c->u0 = c->cur; c->cur = 1 - c->cur; }
-  c->halo_prim[0] = c->halo_prim[1] = false;   // the new primitives have no external ghost planes yet
+  // the new primitives have no external ghost planes yet -- except on a side with a mapped neighbour, whose own
+  // substep stores them (hz_peer_attach: mutual, lockstep)
+  for (int s = 0; s < 2; s++) c->halo_prim[s] = c->peer_P[s][0] != nullptr;
   c->pcur = 1 - c->pcur;
   c->stage = (st + 1) % 3;
   return HZ_OK;
@@ -379,6 +411,12 @@ int make_maps_tr(hz_ctx* c) {
       cudaFuncSetAttribute(k_substep<float, double, R, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)TileGeom<float, R>::SMEM) != cudaSuccess ||
       cudaFuncSetAttribute(k_substep<float, double, R, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)TileGeom<float, R>::SMEM) != cudaSuccess) {
+    cudaGetLastError();
+    return HZ_ECUDA;
+  }
+  if (cudaFuncSetAttribute(k_substep<T, T, R, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(k_substep<float, double, R, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)TileGeom<float, R>::SMEM) != cudaSuccess) {
     cudaGetLastError();
     return HZ_ECUDA;
@@ -588,6 +626,8 @@ int hz_create(const hz_grid* grid, int dtype, const hz_params* params, void* dev
   c->cur = 0; c->u0 = 1; c->pcur = 0; c->stage = 0;
   c->have_metric = c->have_prim = false;
   c->halo_met[0] = c->halo_met[1] = c->halo_prim[0] = c->halo_prim[1] = false;
+  c->peer_P[0][0] = c->peer_P[0][1] = c->peer_P[1][0] = c->peer_P[1][1] = nullptr;
+  c->peer_fs[0] = c->peer_fs[1] = 0; c->peer_nz[0] = c->peer_nz[1] = 0;
   c->launches = 0;
   c->prof = false;
   c->gexec = nullptr; c->gstream = nullptr; c->gev[0] = c->gev[1] = nullptr;
@@ -709,6 +749,32 @@ int hz_halo_unpack(hz_ctx* c, int which, int side, const void* device_buf) {
   if (!device_buf || !is_device_ptr(device_buf)) return HZ_EINVAL;
   const int k0 = side == 0 ? 0 : c->L.g[2] + c->L.n[2];
   return HZ_DISPATCH(c, halo_copy_t, c, which, k0, const_cast<void*>(device_buf), 1);
+}
+
+int hz_prim_buffers(hz_ctx* c, void** P0, void** P1, long long* field_stride) {
+  if (!c || !P0 || !P1 || !field_stride) return HZ_EINVAL;
+  if (c->dtype == HZ_F64) { *P0 = c->P<double>(0); *P1 = c->P<double>(1); }
+  else { *P0 = c->P<float>(0); *P1 = c->P<float>(1); }
+  *field_stride = c->L.fs;
+  return HZ_OK;
+}
+
+int hz_peer_attach(hz_ctx* c, int side, void* peer_P0, void* peer_P1, long long peer_field_stride, int peer_nz) {
+  if (!c || (side != 0 && side != 1) || !peer_P0 || !peer_P1 || peer_field_stride <= 0 || peer_nz < c->L.ng) return HZ_EINVAL;
+  if (!side_external(c, side)) return HZ_EINVAL;
+  if (!is_device_ptr(peer_P0) || !is_device_ptr(peer_P1)) return HZ_EINVAL;
+  // the peer stores are compiled into the kernels of the configuration every BASELINE workload runs
+  if (!(c->par.cleaning != 0 && c->par.energy_var == 0) || getenv("HZ_DEBUG_NO_FAST")) return HZ_EINVAL;
+  c->peer_P[side][0] = peer_P0; c->peer_P[side][1] = peer_P1;
+  c->peer_fs[side] = peer_field_stride;
+  c->peer_nz[side] = peer_nz;
+  return HZ_OK;
+}
+
+int hz_peer_detach(hz_ctx* c, int side) {
+  if (!c || (side != 0 && side != 1)) return HZ_EINVAL;
+  c->peer_P[side][0] = c->peer_P[side][1] = nullptr;
+  return HZ_OK;
 }
 
 long long hz_launch_count(const hz_ctx* c) { return c ? c->launches : 0; }

@@ -487,13 +487,37 @@ __device__ __forceinline__ int image_coord(const Layout& L, int d, int c, int t)
   if (L.bc[d] == 0) return (t == 1 && c < L.ng) ? c + n : c - n;
   return c == 0 ? -t : n - 1 + t;
 }
-template <typename T>
+// ---- halo exchange fused into the substep ("peer stores") ----------
+// A slab whose neighbour's primitive buffers are mapped into this process (another context on this GPU, a peer
+// GPU of this process, or a CUDA-IPC mapping of another process's buffer; hz_peer_attach) stores the cells within
+// NG of that cut -- and their x / y ghost images -- straight into the neighbour's ghost planes while it writes its
+// own: no pack kernel, no transfer, no unpack kernel.  dst[s]: the neighbour's primitive set that this substep
+// writes (side s: 0 below, 1 above), 0 = no neighbour mapped; fs[s]: its field stride; nz0: interior planes of the
+// neighbour below.  The two slabs have the same extent in x and y, hence the same row and plane strides.
+template <typename T, int PEER> struct PeerArg {};
+template <typename T> struct PeerArg<T, 1> { T* dst[2]; long long fs[2]; int nz0; };
+
+template <typename T, int PEER = 0>
 __device__ __forceinline__ void store_prims_with_images(const Layout& L, T* __restrict__ Pout, int i, int j, int k,
-                                                        const T* q) {
+                                                        const T* q, const PeerArg<T, PEER>& peer = PeerArg<T, PEER>()) {
   const long long id0 = L.idx(i, j, k);
 #pragma unroll
   for (int v = 0; v < NV; v++) Pout[v * L.fs + id0] = q[v];
   const int ci = image_count(L, 0, i), cj = image_count(L, 1, j), ck = image_count(L, 2, k);
+  if constexpr (PEER) {
+#pragma unroll   // (static index into the kernel parameter: a run-time one would copy it to local memory)
+    for (int s = 0; s < 2; s++) {
+      if (peer.dst[s] == nullptr || !(s == 0 ? k < L.ng : k >= L.n[2] - L.ng)) continue;
+      const int kp = s == 0 ? peer.nz0 + k : k - L.n[2];   // this plane in the neighbour's coordinates: a ghost plane
+      for (int b = 0; b <= cj; b++)
+        for (int a = 0; a <= ci; a++) {
+          const long long id = (long long)(kp + L.g[2]) * L.sz + (long long)(image_coord(L, 1, j, b) + L.g[1]) * L.pitch +
+                               (image_coord(L, 0, i, a) + L.ox);
+#pragma unroll
+          for (int v = 0; v < NV; v++) peer.dst[s][v * peer.fs[s] + id] = q[v];
+        }
+    }
+  }
   if ((ci | cj | ck) == 0) return;   // not within reach of a boundary: the common case
   for (int c = 0; c <= ck; c++)
     for (int b = 0; b <= cj; b++)
@@ -621,12 +645,13 @@ __device__ __forceinline__ void issue_loads(const CUtensorMap* tmP, const CUtens
 // T2 is the arithmetic type of phase 2.  T2 = T: pure fp64 or pure fp32.  T = float with
 // T2 = double is the paper's mixed mode: storage, reconstruction and face fluxes in
 // fp32; flux difference, Runge-Kutta combine and the primitive recovery in fp64.
-template <typename T, typename T2, int R, int FAST>
+// PEER = 1: the instantiation for slabs with mapped neighbours (peer stores, above); `peer` is an empty struct otherwise.
+template <typename T, typename T2, int R, int FAST, int PEER = 0>
 __global__ void __launch_bounds__(Tile<T, R>::NT, 1)
 k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmM, Layout L, Par<T> par,
           Par<T2> par2, const T* __restrict__ cln, const T* Uin, const T* __restrict__ U0, T* Uout,
           T* __restrict__ Pout, int stage, T2 dt, unsigned long long* __restrict__ counters, int ntx, int nty,
-          int ntiles, const int* __restrict__ order) {
+          int ntiles, const int* __restrict__ order, const PeerArg<T, PEER> peer = PeerArg<T, PEER>()) {
   using G = TileGeom<T, R>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* sP = reinterpret_cast<T*>(smem_raw + G::OFF_P);  // sP[field][z][y][x], halo 2 (HX in x)
@@ -830,7 +855,7 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
         Uout[v * L.fs + id] = (T)un[v];
         qs[v] = (T)qn[v];
       }
-      store_prims_with_images(L, Pout, ci, cj, ck, qs);
+      store_prims_with_images<T, PEER>(L, Pout, ci, cj, ck, qs, peer);
     }
   }
   // warp-level reduction of the counters: [0] c2p_fail, [1] atm_reset, [2] p_floor, [3] max iterations,

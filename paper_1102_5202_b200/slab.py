@@ -104,8 +104,13 @@ class DistTransport:
         return self._buf[key]
 
     def exchange(self, slab, which, device="cuda"):
+        import torch
         import torch.distributed as dist
         send, recv = self._buffers(which, slab.hz.halo_bytes(which), device)
+        # gloo cannot send from device memory: with it (the one-GPU tests) the buffers go through the host.  NCCL,
+        # the transport this module is for, sends them as they are.
+        staged = torch.device(device).type == "cuda" and dist.get_backend(self.group) != "nccl"
+        wire_send, wire_recv = ([None, None], [None, None]) if staged else (send, recv)
         # NCCL pairs the sends and receives between two ranks in posting order (it has no tags; none are used
         # here, so gloo in the CPU test matches the same way).  Sends go
         # low side first; receives are posted high side first, because a neighbour's low-side planes land in
@@ -116,11 +121,15 @@ class DistTransport:
             if nb is None:
                 continue
             slab.hz.halo_pack(which, side, send[side])       # on the current stream; NCCL waits for it
-            sends.append(dist.P2POp(dist.isend, send[side], nb, self.group))
+            if staged:
+                wire_send[side] = send[side].cpu()
+            sends.append(dist.P2POp(dist.isend, wire_send[side], nb, self.group))
         for side in (1, 0):
             nb = slab.nb[side]
             if nb is not None:
-                recvs.append(dist.P2POp(dist.irecv, recv[side], nb, self.group))
+                if staged:
+                    wire_recv[side] = torch.empty(recv[side].shape, dtype=torch.uint8)
+                recvs.append(dist.P2POp(dist.irecv, wire_recv[side], nb, self.group))
         if sends or recvs:
             # With NCCL, wait() does not block the host: it makes the current stream wait for the transfer, so
             # the unpack kernels below are ordered behind it on the device and hz_step stays asynchronous.
@@ -129,6 +138,8 @@ class DistTransport:
                 req.wait()
         for side in (0, 1):
             if slab.nb[side] is not None:
+                if staged:
+                    recv[side].copy_(wire_recv[side])
                 slab.hz.halo_unpack(which, side, recv[side])
 
 
@@ -148,6 +159,7 @@ class Slab:
         self.rank, self.parts, self.sl = rank, parts, sl
         self.nb = neighbours(w.bc[2], rank, parts)
         self.ncell = n[0] * n[1] * n[2]
+        self.nz = n[2]
         self.hz = Horizon(n, h, bc, dtype=dtype, params=HzParams.default(**w.params), **kw)
         self._w = w
 
@@ -164,16 +176,27 @@ class Slab:
         torch.cuda.current_stream().synchronize()
 
 
+def attach_neighbours(slabs):
+    """Mutual hz_peer_attach of slabs that live in one process (their buffers are plain device addresses; on
+    several GPUs of one process they are peer-mapped addresses once peer access is enabled)."""
+    for s in slabs:
+        for side in (0, 1):
+            if s.nb[side] is not None:
+                o = slabs[s.nb[side]]
+                p0, p1, fs = o.hz.prim_buffers()
+                s.hz.peer_attach(side, p0, p1, fs, o.nz)
+
+
 class SlabGroup:
     """R slabs in one process on one GPU, stepped in lockstep (validation of the exchange).
     `w`: the global workload, or a list of per-slab workloads (local slabs, see Slab)."""
 
-    def __init__(self, w, parts, dtype="f64"):
-        self.w, self.parts = w, parts
+    def __init__(self, w, parts, dtype="f64", fused=False, **kw):
+        self.w, self.parts, self.fused = w, parts, fused
         if isinstance(w, (list, tuple)):
-            self.slabs = [Slab(w[r], r, parts, dtype, local=True) for r in range(parts)]
+            self.slabs = [Slab(w[r], r, parts, dtype, local=True, **kw) for r in range(parts)]
         else:
-            self.slabs = [Slab(w, r, parts, dtype) for r in range(parts)]
+            self.slabs = [Slab(w, r, parts, dtype, **kw) for r in range(parts)]
         self.tr = LocalTransport()
         for s in self.slabs:
             s.set_metric()
@@ -181,12 +204,18 @@ class SlabGroup:
         for s in self.slabs:
             s.set_primitives()
         self.tr.exchange(self.slabs, HZ_HALO_PRIM)
+        if fused:
+            # fused=True: the exchange of the primitives is part of the substep kernel (hz_peer_attach): every slab
+            # stores its planes next to a cut straight into the neighbour's ghost planes.  All slabs run on one
+            # stream here, so a slab's next substep is ordered behind its neighbours' last one.
+            attach_neighbours(self.slabs)
 
     def substeps(self, dt, nsub):
         for _ in range(nsub):
             for s in self.slabs:
                 s.hz.substeps(dt, 1)
-            self.tr.exchange(self.slabs, HZ_HALO_PRIM)
+            if not self.fused:
+                self.tr.exchange(self.slabs, HZ_HALO_PRIM)
 
     def get_primitives(self):
         return np.concatenate([s.hz.get_primitives() for s in self.slabs], axis=1)
@@ -220,21 +249,65 @@ class DistSlabHorizon:
     scalars.
     """
 
-    def __init__(self, w, dtype="f64", group=None, device="cuda", local=False):
+    def __init__(self, w, dtype="f64", group=None, device="cuda", local=False, fused=False):
         import torch.distributed as dist
         self.rank, self.parts = dist.get_rank(group), dist.get_world_size(group)
-        self.group, self.device = group, device
+        self.group, self.device, self.fused = group, device, fused
         self.slab = Slab(w, self.rank, self.parts, dtype, local=local)
         self.tr = DistTransport(group)
         self.slab.set_metric()
         self.tr.exchange(self.slab, HZ_HALO_METRIC, device)
         self.slab.set_primitives()
         self.tr.exchange(self.slab, HZ_HALO_PRIM, device)
+        if fused:
+            self._attach_over_ipc()
+
+    def _attach_over_ipc(self):
+        """fused=True: the exchange of the primitives as part of the substep kernel across PROCESSES of one node.
+        Every rank exports its state buffer as a CUDA IPC handle, the ranks gather the handles, a rank opens its
+        neighbours' buffers (over NVLink they are peer memory) and attaches them (hz_peer_attach); from then on
+        the only traffic between substeps is a barrier."""
+        import torch
+        import torch.distributed as dist
+        from torch.multiprocessing.reductions import reduce_tensor
+        hz = self.slab.hz
+        p0, p1, fs = hz.prim_buffers()
+        base = hz._buf.data_ptr()
+        mine = dict(ipc=reduce_tensor(hz._buf), off0=p0 - base, off1=p1 - base, fs=fs, nz=self.slab.nz)
+        infos = [None] * self.parts
+        dist.all_gather_object(infos, mine, group=self.group)
+        self._mapped = {}
+        for side in (0, 1):
+            nb = self.slab.nb[side]
+            if nb is None:
+                continue
+            if nb not in self._mapped:
+                rebuild, args = infos[nb]["ipc"]
+                self._mapped[nb] = rebuild(*args)     # the neighbour's state buffer in this process's address space
+            b = self._mapped[nb].data_ptr()
+            hz.peer_attach(side, b + infos[nb]["off0"], b + infos[nb]["off1"], infos[nb]["fs"], infos[nb]["nz"])
+        self._token = torch.zeros(1, device=self.device)
+        self._lockstep()
+
+    def _lockstep(self):
+        """No rank starts substep s + 1 before its neighbours' substep s has stored into its ghost planes.  With NCCL
+        a one-element all-reduce is that barrier ON THE DEVICE (stream-ordered, the host does not wait); other
+        backends (gloo in the one-GPU test) synchronise the stream and meet at a host barrier."""
+        import torch
+        import torch.distributed as dist
+        if dist.get_backend(self.group) == "nccl":
+            dist.all_reduce(self._token, group=self.group)
+        else:
+            torch.cuda.current_stream().synchronize()
+            dist.barrier(group=self.group)
 
     def substeps(self, dt, nsub):
         for _ in range(nsub):
             self.slab.hz.substeps(dt, 1)
-            self.tr.exchange(self.slab, HZ_HALO_PRIM, self.device)
+            if self.fused:
+                self._lockstep()
+            else:
+                self.tr.exchange(self.slab, HZ_HALO_PRIM, self.device)
 
     def step(self, dt, n):
         self.substeps(dt, 3 * n)
@@ -259,6 +332,14 @@ class DistSlabHorizon:
         return out
 
     def close(self):
+        if self.fused:
+            # nobody unmaps a buffer a neighbour may still store into
+            self._lockstep()
+            for side in (0, 1):
+                if self.slab.nb[side] is not None:
+                    self.slab.hz.peer_detach(side)
+            self._mapped = {}
+            self._lockstep()
         self.slab.hz.close()
 
 
@@ -274,7 +355,8 @@ def _time_slabs(n, parts, dtype, steps):
     import workloads as wl
     w = wl.kerr_sweep(n)
     out = {}
-    for name, make in (("single", lambda: Horizon.from_workload(w, dtype=dtype)), ("slabs", lambda: SlabGroup(w, parts, dtype))):
+    for name, make in (("single", lambda: Horizon.from_workload(w, dtype=dtype)), ("slabs", lambda: SlabGroup(w, parts, dtype)),
+                       ("fused", lambda: SlabGroup(w, parts, dtype, fused=True))):
         obj = make()
         run = (lambda k: obj.substeps(w.dt, 3 * k))
         run(2)
@@ -286,7 +368,8 @@ def _time_slabs(n, parts, dtype, steps):
         torch.cuda.synchronize()
         out[name] = w.ncell * 3 * steps / (e0.elapsed_time(e1) * 1e-3)
         obj.close()
-    out.update(n=n, parts=parts, dtype=dtype, steps=steps, slab_over_single=out["slabs"] / out["single"])
+    out.update(n=n, parts=parts, dtype=dtype, steps=steps, slab_over_single=out["slabs"] / out["single"],
+               fused_over_single=out["fused"] / out["single"])
     print(json.dumps(out))
 
 

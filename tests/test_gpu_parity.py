@@ -402,6 +402,74 @@ def test_slab_decomposition_reproduces_the_single_domain_bitwise(make, parts, dt
     grp.close()
 
 
+@pytest.mark.parametrize("make,parts,dtype", [
+    (lambda: wl.alfven_wave(n=(19, 12, 20)), 2, "f64"),     # periodic ring of two: both neighbours are the same slab
+    (lambda: wl.alfven_wave(n=(19, 12, 21)), 3, "f64"),     # uneven slabs, periodic in x and y: ghost images travel too
+    (lambda: wl.kerr_sweep(24), 3, "f64"),                  # outflow ends, curved metric
+    (lambda: wl.kerr_sweep(24), 2, "f32"),
+    (lambda: wl.blast(20), 4, "f32h"),
+    (lambda: dataclasses.replace(wl.alfven_wave(n=(19, 12, 21)),
+                                 params={**wl.alfven_wave(n=(19, 12, 21)).params, "recon": 1}), 3, "f64"),   # PPM: 3 planes
+])
+def test_exchange_fused_into_the_substep_reproduces_the_single_domain_bitwise(make, parts, dtype):
+    """Row f3 / SURVEY 8(e): with the neighbours' primitive buffers attached (hz_peer_attach) the substep kernel
+    stores the planes next to a cut straight into the neighbour's ghost planes -- no pack / unpack launches between
+    substeps -- and the result is the single-context one bit for bit, like the pack / unpack path's."""
+    from paper_1102_5202_b200 import SlabGroup
+    w = make()
+    one = horizon(w, dtype)
+    grp = SlabGroup(w, parts, dtype, fused=True)
+    n0 = sum(s.hz.launch_count() for s in grp.slabs)
+    one.substeps(w.dt, 5)
+    grp.substeps(w.dt, 5)
+    assert sum(s.hz.launch_count() for s in grp.slabs) - n0 == 5 * parts     # nothing but the substep kernels
+    a, b = one.get_primitives(), grp.get_primitives()
+    assert np.array_equal(a, b), f"max |diff| = {np.abs(a - b).max()}"
+    da, db = one.diagnostics(), grp.diagnostics()
+    for k in ("c2p_fail", "atm_reset", "p_floor", "divB_max", "max_speed_over_dx"):
+        assert da[k] == db[k]
+    one.close()
+    grp.close()
+
+
+def test_peer_attach_reports_errors_and_detach_returns_to_pack_unpack():
+    from paper_1102_5202_b200 import SlabGroup
+    from paper_1102_5202_b200 import binding as B
+    w = wl.kerr_sweep(24)
+    one = horizon(w, "f64")
+    p0, p1, fs = one.prim_buffers()
+    assert p0 and p1 and p0 != p1 and fs > 24 ** 3
+    with pytest.raises(B.HzError):            # no external side on a whole domain
+        one.peer_attach(0, p0, p1, fs, 24)
+    grp = SlabGroup(w, 3, "f64", fused=True)
+    lo = grp.slabs[0]
+    with pytest.raises(B.HzError):            # the low side of the lowest slab is the domain's outflow end
+        lo.hz.peer_attach(0, p0, p1, fs, 8)
+    with pytest.raises(B.HzError):            # side out of range
+        lo.hz.peer_attach(2, p0, p1, fs, 8)
+    # the general-mode kernels have no peer stores
+    wg = dataclasses.replace(w, params={**w.params, "energy_var": 1})
+    gg = SlabGroup(wg, 2, "f64")
+    q0, q1, qfs = gg.slabs[1].hz.prim_buffers()
+    with pytest.raises(B.HzError):
+        gg.slabs[0].hz.peer_attach(1, q0, q1, qfs, gg.slabs[1].nz)
+    gg.close()
+    # detached, a slab is back under the rule of hz_halo_unpack: stepping twice without an exchange is refused
+    one.substeps(w.dt, 2)
+    grp.substeps(w.dt, 1)
+    for s in grp.slabs:
+        for side in (0, 1):
+            s.hz.peer_detach(side)
+    grp.fused = False
+    grp.substeps(w.dt, 1)
+    assert np.array_equal(one.get_primitives(), grp.get_primitives())
+    grp.slabs[1].hz.substeps(w.dt, 1)
+    with pytest.raises(B.HzError):
+        grp.slabs[1].hz.substeps(w.dt, 1)
+    one.close()
+    grp.close()
+
+
 def test_halo_calls_report_errors():
     from paper_1102_5202_b200 import binding as B
     import torch
