@@ -269,11 +269,10 @@ class DistSlabHorizon:
         the only traffic between substeps is a barrier."""
         import torch
         import torch.distributed as dist
-        from torch.multiprocessing.reductions import reduce_tensor
         hz = self.slab.hz
         p0, p1, fs = hz.prim_buffers()
         base = hz._buf.data_ptr()
-        mine = dict(ipc=reduce_tensor(hz._buf), off0=p0 - base, off1=p1 - base, fs=fs, nz=self.slab.nz)
+        mine = dict(ipc=self._ipc_export(hz._buf), off0=p0 - base, off1=p1 - base, fs=fs, nz=self.slab.nz)
         infos = [None] * self.parts
         dist.all_gather_object(infos, mine, group=self.group)
         self._mapped = {}
@@ -282,12 +281,22 @@ class DistSlabHorizon:
             if nb is None:
                 continue
             if nb not in self._mapped:
-                rebuild, args = infos[nb]["ipc"]
-                self._mapped[nb] = rebuild(*args)     # the neighbour's state buffer in this process's address space
+                self._mapped[nb] = self._ipc_open(infos[nb]["ipc"])   # the neighbour's state buffer in this address space
             b = self._mapped[nb].data_ptr()
             hz.peer_attach(side, b + infos[nb]["off0"], b + infos[nb]["off1"], infos[nb]["fs"], infos[nb]["nz"])
         self._token = torch.zeros(1, device=self.device)
         self._lockstep()
+
+    @staticmethod
+    def _ipc_export(buf):
+        """A picklable CUDA IPC handle of the tensor `buf` (torch's own: the allocation's handle plus the offset)."""
+        from torch.multiprocessing.reductions import reduce_tensor
+        return reduce_tensor(buf)
+
+    @staticmethod
+    def _ipc_open(blob):
+        rebuild, args = blob
+        return rebuild(*args)
 
     def _lockstep(self):
         """No rank starts substep s + 1 before its neighbours' substep s has stored into its ghost planes.  With NCCL
@@ -298,7 +307,8 @@ class DistSlabHorizon:
         if dist.get_backend(self.group) == "nccl":
             dist.all_reduce(self._token, group=self.group)
         else:
-            torch.cuda.current_stream().synchronize()
+            if torch.device(self.device).type == "cuda":
+                torch.cuda.current_stream().synchronize()
             dist.barrier(group=self.group)
 
     def substeps(self, dt, nsub):

@@ -102,3 +102,73 @@ def test_dist_transport_fills_the_right_ghost_planes(world, bc_z, port):
             assert lo == ([-1.0, -1.0] if rank == 0 else [float(k0 - 2), float(k0 - 1)]), (rank, planes)
             assert hi == ([-1.0, -1.0] if rank == world - 1 else [float(k1), float(k1 + 1)]), (rank, planes)
         assert planes[2:-2] == [float(k) for k in range(k0, k1)]
+
+
+class FakePeerHz:
+    """Stand-in for a context in the fused exchange: records what hz_peer_attach is given."""
+
+    def __init__(self, rank):
+        self._buf = torch.zeros(64, dtype=torch.uint8)
+        self.rank, self.attached, self.detached, self.nsub = rank, {}, [], 0
+
+    def prim_buffers(self):
+        b = self._buf.data_ptr()
+        return b + 8, b + 24, 100 + self.rank
+
+    def peer_attach(self, side, p0, p1, fs, nz):
+        self.attached[side] = (p0, p1, fs, nz)
+
+    def peer_detach(self, side):
+        self.detached.append(side)
+
+    def substeps(self, dt, n):
+        self.nsub += n
+
+    def close(self):
+        pass
+
+
+class FakeMapped:
+    def __init__(self, rank):
+        self.rank = rank
+
+    def data_ptr(self):
+        return 10000 * (self.rank + 1)
+
+
+def _worker_fused(rank, world, port, bc_z, nz, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    d = object.__new__(slab.DistSlabHorizon)           # the rank logic without a GPU context
+    k0, k1 = slab.split_z(nz, world)[rank]
+    sl = type("S", (), {})()
+    sl.hz, sl.nb, sl.nz = FakePeerHz(rank), slab.neighbours(bc_z, rank, world), k1 - k0
+    d.rank, d.parts, d.group, d.device, d.fused, d.slab = rank, world, None, "cpu", True, sl
+    d._ipc_export = lambda buf: ("handle of rank", rank)          # stands in for the CUDA IPC handle
+    d._ipc_open = lambda blob: FakeMapped(blob[1])
+    d._attach_over_ipc()
+    d.substeps(0.1, 3)
+    d.close()
+    out[rank] = (sl.nb, dict(sl.hz.attached), list(sl.hz.detached), sl.hz.nsub)
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,bc_z,port", [(2, B.HZ_BC_PERIODIC, 29745), (3, B.HZ_BC_OUTFLOW, 29746)])
+def test_fused_exchange_attaches_the_right_neighbour_buffers(world, bc_z, port):
+    """DistSlabHorizon(fused=True): every rank exports its buffer, gathers the handles, and attaches to each external
+    side the buffers, field stride and plane count OF THAT SIDE'S NEIGHBOUR (a periodic ring of two attaches the one
+    other rank on both sides); substeps are taken one at a time with a barrier after each; close detaches."""
+    nz = 13
+    sizes = [k1 - k0 for k0, k1 in slab.split_z(nz, world)]
+    with mp.Manager() as man:
+        out = man.dict()
+        mp.spawn(_worker_fused, args=(world, port, bc_z, nz, out), nprocs=world, join=True)
+        res = dict(out)
+    for rank in range(world):
+        nb, attached, detached, nsub = res[rank]
+        assert nsub == 3
+        assert sorted(attached) == [s for s in (0, 1) if nb[s] is not None] == sorted(detached)
+        for side, (p0, p1, fs, pnz) in attached.items():
+            o = nb[side]
+            assert (p0, p1, fs, pnz) == (10000 * (o + 1) + 8, 10000 * (o + 1) + 24, 100 + o, sizes[o]), (rank, side)
