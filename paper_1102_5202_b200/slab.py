@@ -11,6 +11,9 @@ Two transports:
   * DistTransport  -- one process per GPU (torchrun), neighbours exchanged with batched isend/irecv;
   * LocalTransport -- all slabs in ONE process on one GPU, buffers handed over directly.  This is how the
     exchange is validated on a single B200: R slabs must reproduce the single-context run bitwise.
+And no transport at all (fused=True): the neighbours' primitive buffers are attached to each context
+(hz_peer_attach; between processes through CUDA IPC) and the substep kernel itself stores the planes next to a cut
+into the neighbour's ghost planes -- between substeps there is one barrier and no kernel.
 """
 import numpy as np
 
