@@ -583,35 +583,36 @@ __device__ __forceinline__ void face_task(const Layout& L, const Par<T>& par, co
   // face coordinates inside the tile: f = (c * e1 + b) * e0 + a with e0 = TX (+1 for x faces),
   // e1 = TY (+1 for y faces); the quotients by multiply-shift (d is a run-time value here)
   const int e0 = G::TX + (d == 0), e1 = G::TY + (d == 1);
-#if HZ_FACE_ORDER
-  // Which face a lane takes.  The faces of a direction are numbered so that a warp item is whole rows of TX faces
-  // and a (half-)warp takes rows b, b + 2 of ONE plane (swz below): the faces with a < TX and b < TY first, as the
-  // cells are (f < NC), then the TY * TZ x faces with a = TX or the TX * TZ y faces with b = TY.  (Numbered along
+  // Which face a lane takes.  MC tiles: the faces of a direction are numbered so that a warp item is whole rows of TX
+  // faces and a (half-)warp takes rows b, b + 2 of ONE plane (swz below): the faces with a < TX and b < TY first, as
+  // the cells are (f < NC), then the TY * TZ x faces with a = TX or the TX * TZ y faces with b = TY.  (Numbered along
   // rows of TX + 1 x faces or planes of TY + 1 y rows, the rows drifted against the half-warps: the x and y items
-  // took 1.76 shared-memory wavefronts per ideal one.)
+  // took 1.76 shared-memory wavefronts per ideal one.)  The PPM tiles keep the plain numbering: their fp32 box rows
+  // are 16 words, and an item of a = TX faces alone would hit two banks (measured: -6 %).
   int a, b0, c;
-  if (d == 2 || f < G::NC) {
-    const int r = cdiv<G::TX, G::NF>(f);
-    a = f - r * G::TX;
-    c = cdiv<G::TY, G::NF>(r);
-    b0 = r - c * G::TY;
-  } else if (d == 0) {
-    const int g = f - G::NC;
-    a = G::TX;
-    c = cdiv<G::TY, G::NF>(g);
-    b0 = g - c * G::TY;
+  if (HZ_FACE_ORDER && R == 0) {
+    if (d == 2 || f < G::NC) {
+      const int r = cdiv<G::TX, G::NF>(f);
+      a = f - r * G::TX;
+      c = cdiv<G::TY, G::NF>(r);
+      b0 = r - c * G::TY;
+    } else if (d == 0) {
+      const int g = f - G::NC;
+      a = G::TX;
+      c = cdiv<G::TY, G::NF>(g);
+      b0 = g - c * G::TY;
+    } else {
+      const int g = f - G::NC;
+      c = cdiv<G::TX, G::NF>(g);
+      a = g - c * G::TX;
+      b0 = G::TY;
+    }
   } else {
-    const int g = f - G::NC;
-    c = cdiv<G::TX, G::NF>(g);
-    a = g - c * G::TX;
-    b0 = G::TY;
+    const int r = d == 0 ? cdiv<G::TX + 1, G::NF>(f) : cdiv<G::TX, G::NF>(f);
+    a = f - r * e0;
+    c = d == 1 ? cdiv<G::TY + 1, G::NF>(r) : cdiv<G::TY, G::NF>(r);
+    b0 = r - c * e1;
   }
-#else
-  const int r = d == 0 ? cdiv<G::TX + 1, G::NF>(f) : cdiv<G::TX, G::NF>(f);
-  const int a = f - r * e0;
-  const int c = d == 1 ? cdiv<G::TY + 1, G::NF>(r) : cdiv<G::TY, G::NF>(r);
-  const int b0 = r - c * e1;
-#endif
   const int b = b0 < (G::TY & ~3) ? swz(b0) : b0;   // the extra y face (b0 = TY) keeps its row
   // the face lies between cell (a,b,c) - e_d and cell (a,b,c)
   const bool valid = x0 + a < L.n[0] + (d == 0) && y0 + b < L.n[1] + (d == 1) && z0 + c < L.n[2] + (d == 2);
