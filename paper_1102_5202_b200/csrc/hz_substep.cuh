@@ -739,12 +739,11 @@ k_substep(const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUten
       // assignment that minimises the longest warp for fixed item durations leaves two warps with source items only:
       // -16 %; handing a warp consecutive items, all of one sweep axis: -10 %.)
       const int warp = threadIdx.x >> 5;
-      if (warp < 4) {
+      // (one call site for both halves: a second one would put a second copy of the z face body into the kernel)
+      const int t0 = warp < 4 ? warp : 16 + warp, t1 = warp < 4 ? 20 : 28;
 #pragma unroll 1
-        for (int t = warp; t < 20; t += 4) face_task<T, R, FAST>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
-      } else {
-#pragma unroll 1
-        for (int t = 16 + warp; t < 28; t += 4) face_task<T, R, FAST>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
+      for (int t = t0; t < t1; t += 4) face_task<T, R, FAST>(L, par, sP, sM, sF, t, lane, x0, y0, z0);
+      if (warp >= 4) {
 #pragma unroll 1
         for (int t = warp - 4; t < 8; t += 4) source_task<T, R, FAST>(L, par, sP, sM, sR, cln, t * 32 + lane, x0, y0, z0);
       }
